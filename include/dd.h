@@ -1,0 +1,148 @@
+/*
+ * dd.h -- C ABI of libdd.so: brute-force incoherent dedispersion on one B200 (sm_100a).
+ *
+ * What the library computes (arXiv 2311.05341; line numbers are /root/reference/PAPER.md):
+ *
+ *   out[d][t] = sum_{c=0}^{nchans-1} in[c][t + s(d,c)]          Eq. 3, Alg. 1 (72-76)
+ *   s(d,c)    = rint( DM_d * C_DM * (1/f_c^2 - 1/f_high^2) / tsamp )   Eq. 1 (26-30), Eq. 7 (183-188)
+ *   f_c       = f_high + c * chan_bw   (chan_bw < 0: channel 0 is the highest frequency)
+ *   out_len   = nsamps - max_{d,c} s(d,c)   (the same for every DM trial)
+ *
+ * C_DM = 4148.808 MHz^2 s pc^-1 cm^3; shifts are evaluated in IEEE double, rounded
+ * half-to-even.  Integer inputs (uint8, uint16) give exact uint32 sums; float32 input gives
+ * float32 sums (summation order unspecified).  No division by nchans (Alg. 2's last line,
+ * PAPER.md:120, is dropped).  Readings of the paper are listed in DESIGN.md.
+ *
+ * All functions return DD_OK (0) or a negative dd_status; none throws, none prints.
+ * Pointers are HOST pointers unless the name starts with d_ (DEVICE pointer on the plan's
+ * device).  The library never takes ownership of a caller's buffer.
+ * There is no CPU fallback: without a CUDA device of compute capability 10.x,
+ * dd_plan_create fails with DD_ERR_UNSUPPORTED_DEVICE / DD_ERR_CUDA.
+ */
+#ifndef DD_H_
+#define DD_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dd_plan dd_plan;
+
+/* in_dtype of dd_plan_create */
+enum { DD_U8 = 0, DD_U16 = 1, DD_F32 = 2 };
+
+typedef enum dd_status {
+    DD_OK = 0,
+    DD_ERR_INVALID_ARG = -1,        /* null pointer, non-positive size, chan_bw >= 0, bad DM ... */
+    DD_ERR_SHIFT_TOO_LARGE = -2,    /* max shift >= nsamps: no output sample is complete */
+    DD_ERR_OVERFLOW = -3,           /* nchans * max sample value does not fit uint32 */
+    DD_ERR_ALLOC = -4,              /* host or device allocation failed */
+    DD_ERR_CUDA = -5,               /* a CUDA runtime call or kernel launch failed */
+    DD_ERR_UNSUPPORTED_DEVICE = -6, /* current device is not sm_100 (B200) */
+    DD_ERR_UNSUPPORTED_PLAN = -7    /* a single DM trial's staged window exceeds shared memory */
+} dd_status;
+
+/*
+ * Host delay-table builder (Eq. 1 / Eq. 7).  Pure host code, needs
+ * no GPU.  Writes table[d*nchans + c] = s(d,c) (row-major, DM major) and the largest entry
+ * to *max_shift (may be NULL).
+ *   nchans > 0, ndm > 0, f_high_MHz > 0, chan_bw_MHz < 0, f_high + (nchans-1)*chan_bw > 0,
+ *   tsamp_s > 0, every DM finite and >= 0; otherwise DD_ERR_INVALID_ARG.
+ *   A shift that does not fit int32 gives DD_ERR_SHIFT_TOO_LARGE.
+ * `table` is caller-owned, ndm*nchans int32.
+ */
+int dd_shift_table_build(int nchans, double f_high_MHz, double chan_bw_MHz, double tsamp_s,
+                         const double *dm_list, int ndm, int32_t *table, int32_t *max_shift);
+
+/*
+ * Create a plan on the CURRENT CUDA device.  Copies dm_list; builds and owns the host shift
+ * table, its device-side tiling metadata and a device workspace (the lane-interleaved copy
+ * of one input block).  Launches no kernel on the data path.
+ *   in_dtype: DD_U8 / DD_U16 / DD_F32.
+ * Errors (with *out = NULL): DD_ERR_INVALID_ARG (as dd_shift_table_build, plus out == NULL,
+ * nsamps <= 0, unknown dtype); DD_ERR_SHIFT_TOO_LARGE (max shift >= nsamps);
+ * DD_ERR_OVERFLOW (u8: 255*nchans >= 2^32; u16: 65535*nchans >= 2^32); DD_ERR_ALLOC;
+ * DD_ERR_CUDA; DD_ERR_UNSUPPORTED_DEVICE; DD_ERR_UNSUPPORTED_PLAN.
+ */
+int dd_plan_create(dd_plan **out, int nchans, int64_t nsamps, double f_high_MHz,
+                   double chan_bw_MHz, double tsamp_s, const double *dm_list, int ndm,
+                   int in_dtype);
+
+/*
+ * The plan's shift table.  *table points into plan-owned HOST memory ([ndm*nchans] int32,
+ * row-major, DM major), valid until dd_plan_destroy.  Any out-pointer may be NULL.
+ */
+int dd_plan_shift_table(const dd_plan *plan, const int32_t **table, int64_t *out_len,
+                        int32_t *max_shift);
+
+/*
+ * Run the transform (Eq. 3) once.
+ *   d_in : DEVICE, dense [nchans][nsamps] of the plan's in_dtype, time contiguous
+ *          (PAPER.md:114, 163-165).  Any alignment is accepted; rows that are not 4-byte
+ *          aligned take a slower scalar path in the lane-interleave pre-pass.
+ *   d_out: DEVICE, dense [ndm][out_len]; uint32 for DD_U8 / DD_U16, float32 for DD_F32
+ *          (PAPER.md:110-115, 157).  Every element is overwritten.
+ *   cuda_stream: a cudaStream_t (NULL = the legacy default stream).
+ * Asynchronous on that stream: no allocation, no synchronisation, no host read of the data.
+ * The plan's workspace is used by the call, so executions of ONE plan must be ordered on
+ * one stream (or otherwise serialised by the caller); different plans are independent.
+ * Errors: DD_ERR_INVALID_ARG (null plan / pointers), DD_ERR_CUDA (launch failure).
+ */
+int dd_execute(const dd_plan *plan, const void *d_in, void *d_out, void *cuda_stream);
+
+/*
+ * The same transform with HOST buffers: h_in [nchans][nsamps], h_out [ndm][out_len].
+ * Copies h_in to a plan-owned device buffer, runs dd_execute, copies the result back and
+ * waits for the stream.  Buffers should be page-locked for full PCIe bandwidth (pageable
+ * memory works, slower).  The device buffers are allocated on first use and kept until
+ * dd_plan_destroy.  Errors as dd_execute, plus DD_ERR_ALLOC.
+ */
+int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream);
+
+/*
+ * Facts about the plan, for tests and the benchmark.  `what` is one of DD_INFO_*; unknown
+ * keys return -1.
+ */
+enum {
+    DD_INFO_D_DM = 0,          /* DM trials per thread block */
+    DD_INFO_D_J = 1,           /* 32-bit words of the interleaved time axis per thread block */
+    DD_INFO_LANES = 2,         /* samples per 32-bit word: 4 (u8), 2 (u16), 1 (f32) */
+    DD_INFO_L = 3,             /* lane stride L: word j, lane k holds in[c][k*L + j] */
+    DD_INFO_SMEM_BYTES = 4,    /* dynamic shared memory per thread block */
+    DD_INFO_GRID = 5,          /* thread blocks of the main kernel */
+    DD_INFO_THREADS = 6,       /* threads per block of the main kernel */
+    DD_INFO_WORKSPACE_BYTES = 7, /* device workspace owned by the plan */
+    DD_INFO_STAGE_BYTES = 8,   /* bytes the main kernel stages global->shared per launch */
+    DD_INFO_LAUNCHES = 9,      /* kernels dd_execute launches */
+    DD_INFO_CH = 10,           /* channels per pipeline stage */
+    DD_INFO_NSTAGE = 11        /* pipeline stages */
+};
+int64_t dd_plan_info(const dd_plan *plan, int what);
+
+/*
+ * Per-kernel device timing for the benchmark's roofline line.  dd_plan_set_timing(plan, 1)
+ * makes every later dd_execute record CUDA events around its two kernels on the launch
+ * stream (a ring of the last 64 executions; a few microseconds of host time per call);
+ * dd_plan_set_timing(plan, 0) stops that.  dd_plan_kernel_times waits for the most recent
+ * timed execution, writes the durations (milliseconds) of up to max_n of the latest timed
+ * executions, oldest first, to interleave_ms[] / main_ms[] (either may be NULL) and returns
+ * how many it wrote (0 if none), or a negative dd_status.
+ */
+int dd_plan_set_timing(dd_plan *plan, int on);
+int dd_plan_kernel_times(dd_plan *plan, int max_n, float *interleave_ms, float *main_ms);
+
+/* Frees everything the plan owns (waits for the device first).  NULL is a no-op. */
+void dd_plan_destroy(dd_plan *plan);
+
+/* Static, never-NULL description of a dd_status value. */
+const char *dd_strerror(int status);
+
+/* Library version string, e.g. "dd 0.1 sm_100a". */
+const char *dd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DD_H_ */

@@ -1,0 +1,213 @@
+"""Thin ctypes face of libdd.so (include/dd.h).  Argument marshalling only: every step of
+the transform runs in the library's CUDA kernels.  PyTorch appears only as the owner of
+device memory and streams.  There is no CPU fallback -- a missing library or a missing
+GPU raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libdd.so")
+
+DD_U8, DD_U16, DD_F32 = 0, 1, 2
+DD_OK = 0
+DD_ERR_INVALID_ARG = -1
+DD_ERR_SHIFT_TOO_LARGE = -2
+DD_ERR_OVERFLOW = -3
+DD_ERR_ALLOC = -4
+DD_ERR_CUDA = -5
+DD_ERR_UNSUPPORTED_DEVICE = -6
+DD_ERR_UNSUPPORTED_PLAN = -7
+
+INFO = {"D_DM": 0, "D_J": 1, "LANES": 2, "L": 3, "SMEM_BYTES": 4, "GRID": 5, "THREADS": 6,
+        "WORKSPACE_BYTES": 7, "STAGE_BYTES": 8, "LAUNCHES": 9, "CH": 10, "NSTAGE": 11}
+
+# every symbol include/dd.h declares (tests check the .so exports all of them)
+SYMBOLS = ("dd_shift_table_build", "dd_plan_create", "dd_plan_shift_table", "dd_execute",
+           "dd_execute_host", "dd_plan_info", "dd_plan_set_timing", "dd_plan_kernel_times",
+           "dd_plan_destroy", "dd_strerror", "dd_version")
+
+_lib = None
+
+
+class DDError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__("%s: %s (dd_status %d)" % (where, strerror(status), status))
+
+
+def lib() -> ctypes.CDLL:
+    """Load libdd.so.  Raises if it has not been built (python -m paper_2311_05341_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("libdd.so is not built: run `python -m paper_2311_05341_b200.build` "
+                              "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        c = ctypes
+        L.dd_shift_table_build.restype = c.c_int
+        L.dd_shift_table_build.argtypes = [c.c_int, c.c_double, c.c_double, c.c_double,
+                                           c.c_void_p, c.c_int, c.c_void_p, c.c_void_p]
+        L.dd_plan_create.restype = c.c_int
+        L.dd_plan_create.argtypes = [c.POINTER(c.c_void_p), c.c_int, c.c_int64, c.c_double,
+                                     c.c_double, c.c_double, c.c_void_p, c.c_int, c.c_int]
+        L.dd_plan_shift_table.restype = c.c_int
+        L.dd_plan_shift_table.argtypes = [c.c_void_p, c.POINTER(c.c_void_p),
+                                          c.POINTER(c.c_int64), c.POINTER(c.c_int32)]
+        L.dd_execute.restype = c.c_int
+        L.dd_execute.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p]
+        L.dd_execute_host.restype = c.c_int
+        L.dd_execute_host.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p]
+        L.dd_plan_info.restype = c.c_int64
+        L.dd_plan_info.argtypes = [c.c_void_p, c.c_int]
+        L.dd_plan_set_timing.restype = c.c_int
+        L.dd_plan_set_timing.argtypes = [c.c_void_p, c.c_int]
+        L.dd_plan_kernel_times.restype = c.c_int
+        L.dd_plan_kernel_times.argtypes = [c.c_void_p, c.c_int, c.c_void_p, c.c_void_p]
+        L.dd_plan_destroy.restype = None
+        L.dd_plan_destroy.argtypes = [c.c_void_p]
+        L.dd_strerror.restype = c.c_char_p
+        L.dd_strerror.argtypes = [c.c_int]
+        L.dd_version.restype = c.c_char_p
+        L.dd_version.argtypes = []
+        _lib = L
+    return _lib
+
+
+def strerror(status: int) -> str:
+    return lib().dd_strerror(int(status)).decode()
+
+
+def version() -> str:
+    return lib().dd_version().decode()
+
+
+def _dm_array(dm_list) -> np.ndarray:
+    return np.ascontiguousarray(dm_list, dtype=np.float64)
+
+
+def dd_shift_table_build(nchans, f_high_MHz, chan_bw_MHz, tsamp_s, dm_list):
+    """Host delay table (no GPU needed).  Returns (int32 [ndm, nchans], max_shift)."""
+    dm = _dm_array(dm_list)
+    table = np.empty((dm.size, max(int(nchans), 0)), dtype=np.int32)
+    mx = ctypes.c_int32(0)
+    rc = lib().dd_shift_table_build(int(nchans), float(f_high_MHz), float(chan_bw_MHz),
+                                    float(tsamp_s), dm.ctypes.data, int(dm.size),
+                                    table.ctypes.data, ctypes.addressof(mx))
+    if rc != DD_OK:
+        raise DDError(rc, "dd_shift_table_build")
+    return table, int(mx.value)
+
+
+class Plan:
+    """dd_plan_create / dd_plan_shift_table / dd_execute / dd_plan_destroy with the same
+    argument order as the C ABI."""
+
+    def __init__(self, nchans, nsamps, f_high_MHz, chan_bw_MHz, tsamp_s, dm_list, in_dtype):
+        dm = _dm_array(dm_list)
+        h = ctypes.c_void_p()
+        rc = lib().dd_plan_create(ctypes.byref(h), int(nchans), int(nsamps), float(f_high_MHz),
+                                  float(chan_bw_MHz), float(tsamp_s), dm.ctypes.data,
+                                  int(dm.size), int(in_dtype))
+        if rc != DD_OK:
+            raise DDError(rc, "dd_plan_create")
+        self._h = h
+        self.nchans, self.nsamps, self.ndm, self.in_dtype = int(nchans), int(nsamps), int(dm.size), int(in_dtype)
+        tab = ctypes.c_void_p()
+        out_len = ctypes.c_int64()
+        mx = ctypes.c_int32()
+        rc = lib().dd_plan_shift_table(self._h, ctypes.byref(tab), ctypes.byref(out_len),
+                                       ctypes.byref(mx))
+        if rc != DD_OK:
+            raise DDError(rc, "dd_plan_shift_table")
+        self.out_len, self.max_shift = int(out_len.value), int(mx.value)
+        self._table_ptr = tab.value
+
+    # -- dd_plan_shift_table
+    def shift_table(self) -> np.ndarray:
+        """A copy of the plan's host table, int32 [ndm, nchans]."""
+        n = self.ndm * self.nchans
+        buf = (ctypes.c_int32 * n).from_address(self._table_ptr)
+        return np.frombuffer(buf, dtype=np.int32).reshape(self.ndm, self.nchans).copy()
+
+    def info(self, key: str) -> int:
+        return int(lib().dd_plan_info(self._h, INFO[key]))
+
+    # -- dd_execute
+    def execute(self, d_in, d_out, stream=None) -> None:
+        """d_in / d_out: torch CUDA tensors (dense) or raw device addresses (int)."""
+        rc = lib().dd_execute(self._h, _dev_ptr(d_in), _dev_ptr(d_out), _stream_ptr(stream))
+        if rc != DD_OK:
+            raise DDError(rc, "dd_execute")
+
+    # -- dd_execute_host
+    def execute_host(self, h_in, h_out, stream=None) -> None:
+        """h_in / h_out: host buffers (numpy arrays or CPU torch tensors, ideally pinned)."""
+        rc = lib().dd_execute_host(self._h, _host_ptr(h_in), _host_ptr(h_out), _stream_ptr(stream))
+        if rc != DD_OK:
+            raise DDError(rc, "dd_execute_host")
+
+    # -- dd_plan_set_timing / dd_plan_kernel_times
+    def set_timing(self, on: bool) -> None:
+        rc = lib().dd_plan_set_timing(self._h, 1 if on else 0)
+        if rc != DD_OK:
+            raise DDError(rc, "dd_plan_set_timing")
+
+    def kernel_times(self, max_n: int = 64):
+        """(interleave_ms[], main_ms[]) of the latest timed executions, oldest first."""
+        a = np.zeros(max_n, dtype=np.float32)
+        b = np.zeros(max_n, dtype=np.float32)
+        n = lib().dd_plan_kernel_times(self._h, int(max_n), a.ctypes.data, b.ctypes.data)
+        if n < 0:
+            raise DDError(n, "dd_plan_kernel_times")
+        return a[:n].copy(), b[:n].copy()
+
+    def destroy(self) -> None:
+        if getattr(self, "_h", None) is not None and self._h:
+            lib().dd_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+
+def _dev_ptr(x) -> int:
+    if isinstance(x, int):
+        return x
+    if not x.is_cuda or not x.is_contiguous():
+        raise ValueError("dd_execute wants dense CUDA tensors")
+    return x.data_ptr()
+
+
+def _host_ptr(x) -> int:
+    if isinstance(x, int):
+        return x
+    if isinstance(x, np.ndarray):
+        if not x.flags.c_contiguous:
+            raise ValueError("host buffer must be C-contiguous")
+        return x.ctypes.data
+    if x.is_cuda or not x.is_contiguous():
+        raise ValueError("dd_execute_host wants dense host tensors")
+    return x.data_ptr()
+
+
+def _stream_ptr(stream) -> int:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream

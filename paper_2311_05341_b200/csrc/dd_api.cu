@@ -1,0 +1,335 @@
+// dd_api.cu -- the C ABI of libdd.so (include/dd.h): plan lifetime, launches, host-buffer path.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "dd_internal.h"
+
+struct dd_plan {
+    int nchans = 0, ndm = 0, in_dtype = 0, device = -1;
+    int64_t nsamps = 0, out_len = 0;
+    int32_t max_shift = 0;
+    double f_high = 0, chan_bw = 0, tsamp = 0;
+    std::vector<double> dm_list;
+    std::vector<int32_t> table;  // [ndm][nchans]
+    dd::Tiling til;
+    // device
+    uint32_t *d_X = nullptr;
+    int32_t *d_ofs = nullptr, *d_base = nullptr, *d_len = nullptr;
+    int64_t workspace_bytes = 0;
+    // dd_execute_host buffers (lazy)
+    void *d_in_own = nullptr, *d_out_own = nullptr;
+    // optional per-kernel timing (dd_plan_set_timing): ring of event triples
+    static constexpr int kRing = 64;
+    bool timing = false;
+    cudaEvent_t ev[kRing][3] = {};
+    bool ev_made = false;
+    mutable int64_t timed_count = 0;
+};
+
+namespace {
+
+size_t elem_bytes(int dtype) { return dtype == DD_U8 ? 1 : (dtype == DD_U16 ? 2 : 4); }
+
+void free_device(dd_plan *p)
+{
+    if (p->device >= 0) {
+        int cur = -1;
+        cudaGetDevice(&cur);
+        if (cur != p->device) cudaSetDevice(p->device);
+        cudaDeviceSynchronize();
+        cudaFree(p->d_X);
+        cudaFree(p->d_ofs);
+        cudaFree(p->d_base);
+        cudaFree(p->d_len);
+        cudaFree(p->d_in_own);
+        cudaFree(p->d_out_own);
+        if (p->ev_made)
+            for (auto &triple : p->ev)
+                for (cudaEvent_t e : triple) cudaEventDestroy(e);
+        if (cur >= 0 && cur != p->device) cudaSetDevice(cur);
+    }
+}
+
+template <typename T>
+int upload(T **dst, const std::vector<T> &src)
+{
+    if (cudaMalloc(reinterpret_cast<void **>(dst), src.size() * sizeof(T)) != cudaSuccess) {
+        cudaGetLastError();
+        return DD_ERR_ALLOC;
+    }
+    if (cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice) != cudaSuccess)
+        return DD_ERR_CUDA;
+    return DD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int dd_shift_table_build(int nchans, double f_high_MHz, double chan_bw_MHz, double tsamp_s,
+                         const double *dm_list, int ndm, int32_t *table, int32_t *max_shift)
+{
+    return dd::build_shift_table(nchans, f_high_MHz, chan_bw_MHz, tsamp_s, dm_list, ndm, table,
+                                 max_shift);
+}
+
+int dd_plan_create(dd_plan **out, int nchans, int64_t nsamps, double f_high_MHz,
+                   double chan_bw_MHz, double tsamp_s, const double *dm_list, int ndm,
+                   int in_dtype)
+{
+    if (!out) return DD_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!dm_list || nchans <= 0 || ndm <= 0 || nsamps <= 0) return DD_ERR_INVALID_ARG;
+    if (in_dtype != DD_U8 && in_dtype != DD_U16 && in_dtype != DD_F32) return DD_ERR_INVALID_ARG;
+    // exact uint32 sums (Heimdall's overflow beyond 8192 channels)
+    const uint64_t top = in_dtype == DD_U8 ? 255u : 65535u;
+    if (in_dtype != DD_F32 && top * static_cast<uint64_t>(nchans) >= (1ull << 32))
+        return DD_ERR_OVERFLOW;
+
+    dd_plan *p = new (std::nothrow) dd_plan;
+    if (!p) return DD_ERR_ALLOC;
+    int rc = DD_OK;
+    try {
+        p->nchans = nchans;
+        p->ndm = ndm;
+        p->nsamps = nsamps;
+        p->in_dtype = in_dtype;
+        p->f_high = f_high_MHz;
+        p->chan_bw = chan_bw_MHz;
+        p->tsamp = tsamp_s;
+        p->dm_list.assign(dm_list, dm_list + ndm);
+        p->table.resize(static_cast<size_t>(ndm) * nchans);
+        rc = dd::build_shift_table(nchans, f_high_MHz, chan_bw_MHz, tsamp_s, p->dm_list.data(), ndm,
+                                   p->table.data(), &p->max_shift);
+        if (rc == DD_OK && p->max_shift >= nsamps) rc = DD_ERR_SHIFT_TOO_LARGE;
+        if (rc != DD_OK) {
+            delete p;
+            return rc;
+        }
+        p->out_len = nsamps - p->max_shift;
+
+        // ---- device
+        int dev = -1;
+        cudaDeviceProp prop;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+            cudaGetLastError();
+            delete p;
+            return DD_ERR_CUDA;
+        }
+        if (prop.major != 10) {
+            delete p;
+            return DD_ERR_UNSUPPORTED_DEVICE;
+        }
+        p->device = dev;
+        const int64_t smem_limit = static_cast<int64_t>(prop.sharedMemPerBlockOptin);
+
+        // first compiled variant of this dtype whose shared-memory ring fits
+        bool found = false;
+        for (int v = 0; v < dd::num_variants() && !found; ++v) {
+            const dd::KernelShape &sh = dd::variant_shape(v);
+            if (sh.mode != in_dtype) continue;
+            found = dd::build_tiling(sh, v, p->table.data(), ndm, nchans, p->out_len, p->max_shift,
+                                     smem_limit, &p->til);
+        }
+        if (!found) {
+            p->device = -1;
+            delete p;
+            return DD_ERR_UNSUPPORTED_PLAN;
+        }
+        const dd::Tiling &t = p->til;
+        if (dd::variant_prepare(t.variant, static_cast<int>(t.smem_bytes)) != 0) rc = DD_ERR_CUDA;
+        const size_t xbytes = static_cast<size_t>(t.nch_pad) * t.Lw * 4;
+        if (rc == DD_OK && cudaMalloc(reinterpret_cast<void **>(&p->d_X), xbytes) != cudaSuccess) {
+            cudaGetLastError();
+            rc = DD_ERR_ALLOC;
+        }
+        // padding channel rows stay zero for the life of the plan
+        if (rc == DD_OK && cudaMemset(p->d_X, 0, xbytes) != cudaSuccess) rc = DD_ERR_CUDA;
+        if (rc == DD_OK) rc = upload(&p->d_ofs, t.ofs);
+        if (rc == DD_OK) rc = upload(&p->d_base, t.blk_base);
+        if (rc == DD_OK) rc = upload(&p->d_len, t.blk_len);
+        if (rc == DD_OK && cudaDeviceSynchronize() != cudaSuccess) rc = DD_ERR_CUDA;
+        p->workspace_bytes = static_cast<int64_t>(xbytes) +
+                             static_cast<int64_t>((t.ofs.size() + t.blk_base.size() + t.blk_len.size()) * 4);
+        // the host copies of the tiling tables are no longer needed
+        std::vector<int32_t>().swap(p->til.ofs);
+        std::vector<int32_t>().swap(p->til.blk_base);
+        std::vector<int32_t>().swap(p->til.blk_len);
+    } catch (const std::bad_alloc &) {
+        rc = DD_ERR_ALLOC;
+    }
+    if (rc != DD_OK) {
+        cudaGetLastError();
+        free_device(p);
+        delete p;
+        return rc;
+    }
+    *out = p;
+    return DD_OK;
+}
+
+int dd_plan_shift_table(const dd_plan *plan, const int32_t **table, int64_t *out_len,
+                        int32_t *max_shift)
+{
+    if (!plan) return DD_ERR_INVALID_ARG;
+    if (table) *table = plan->table.data();
+    if (out_len) *out_len = plan->out_len;
+    if (max_shift) *max_shift = plan->max_shift;
+    return DD_OK;
+}
+
+int dd_execute(const dd_plan *plan, const void *d_in, void *d_out, void *cuda_stream)
+{
+    if (!plan || !d_in || !d_out) return DD_ERR_INVALID_ARG;
+    const dd::Tiling &t = plan->til;
+    dd::InterleaveParams ip;
+    ip.in = d_in;
+    ip.X = plan->d_X;
+    ip.nsamps = plan->nsamps;
+    ip.L = t.L;
+    ip.Lw = t.Lw;
+    ip.nchans = plan->nchans;
+    ip.nchunk = static_cast<int>((t.Lw + 1023) / 1024);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const cudaEvent_t *ev = plan->timing ? plan->ev[plan->timed_count % dd_plan::kRing] : nullptr;
+    if (ev) cudaEventRecord(ev[0], st);
+    if (dd::launch_interleave(plan->in_dtype, ip, cuda_stream) != 0) return DD_ERR_CUDA;
+    if (ev) cudaEventRecord(ev[1], st);
+
+    dd::KernelParams kp;
+    kp.X = plan->d_X;
+    kp.ofs = plan->d_ofs;
+    kp.blk_base = plan->d_base;
+    kp.blk_len = plan->d_len;
+    kp.out = d_out;
+    kp.out_len = plan->out_len;
+    kp.Lw = t.Lw;
+    kp.L = t.L;
+    kp.ndm = plan->ndm;
+    kp.nch_pad = t.nch_pad;
+    kp.nk = t.nk;
+    kp.ndb = t.ndb;
+    kp.ntj = t.ntj;
+    kp.pitch_bytes = t.pitch_words * 4;
+    kp.nstage = t.nstage;
+    kp.stage_bytes = t.shape.CH * t.pitch_words * 4 + t.shape.D_DM() * t.shape.CH * 4;
+    const int grid = t.ndb * t.ntj;
+    if (dd::launch_dedisperse(t.variant, kp, grid, static_cast<int>(t.smem_bytes), cuda_stream) != 0)
+        return DD_ERR_CUDA;
+    if (ev) {
+        cudaEventRecord(ev[2], st);
+        ++plan->timed_count;
+    }
+    return DD_OK;
+}
+
+int dd_plan_set_timing(dd_plan *plan, int on)
+{
+    if (!plan) return DD_ERR_INVALID_ARG;
+    if (on && !plan->ev_made) {
+        for (auto &triple : plan->ev)
+            for (cudaEvent_t &e : triple)
+                if (cudaEventCreate(&e) != cudaSuccess) return DD_ERR_CUDA;
+        plan->ev_made = true;
+    }
+    plan->timing = on != 0;
+    return DD_OK;
+}
+
+int dd_plan_kernel_times(dd_plan *plan, int max_n, float *interleave_ms, float *main_ms)
+{
+    if (!plan || max_n < 0) return DD_ERR_INVALID_ARG;
+    int64_t n = plan->timed_count < dd_plan::kRing ? plan->timed_count : dd_plan::kRing;
+    if (n > max_n) n = max_n;
+    if (n == 0) return 0;
+    const int64_t last = plan->timed_count - 1;
+    if (cudaEventSynchronize(plan->ev[last % dd_plan::kRing][2]) != cudaSuccess) return DD_ERR_CUDA;
+    for (int64_t i = 0; i < n; ++i) {
+        const cudaEvent_t *e = plan->ev[(last - (n - 1) + i) % dd_plan::kRing];
+        float a = 0.f, b = 0.f;
+        if (cudaEventElapsedTime(&a, e[0], e[1]) != cudaSuccess ||
+            cudaEventElapsedTime(&b, e[1], e[2]) != cudaSuccess)
+            return DD_ERR_CUDA;
+        if (interleave_ms) interleave_ms[i] = a;
+        if (main_ms) main_ms[i] = b;
+    }
+    return static_cast<int>(n);
+}
+
+int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream)
+{
+    if (!plan || !h_in || !h_out) return DD_ERR_INVALID_ARG;
+    const size_t in_bytes = static_cast<size_t>(plan->nchans) * plan->nsamps * elem_bytes(plan->in_dtype);
+    const size_t out_bytes = static_cast<size_t>(plan->ndm) * plan->out_len * 4;
+    if (!plan->d_in_own && cudaMalloc(&plan->d_in_own, in_bytes) != cudaSuccess) {
+        cudaGetLastError();
+        plan->d_in_own = nullptr;
+        return DD_ERR_ALLOC;
+    }
+    if (!plan->d_out_own && cudaMalloc(&plan->d_out_own, out_bytes) != cudaSuccess) {
+        cudaGetLastError();
+        plan->d_out_own = nullptr;
+        return DD_ERR_ALLOC;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (cudaMemcpyAsync(plan->d_in_own, h_in, in_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess)
+        return DD_ERR_CUDA;
+    const int rc = dd_execute(plan, plan->d_in_own, plan->d_out_own, cuda_stream);
+    if (rc != DD_OK) return rc;
+    if (cudaMemcpyAsync(h_out, plan->d_out_own, out_bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+        return DD_ERR_CUDA;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return DD_ERR_CUDA;
+    return DD_OK;
+}
+
+int64_t dd_plan_info(const dd_plan *plan, int what)
+{
+    if (!plan) return -1;
+    const dd::Tiling &t = plan->til;
+    switch (what) {
+    case DD_INFO_D_DM: return t.shape.D_DM();
+    case DD_INFO_D_J: return t.shape.D_J();
+    case DD_INFO_LANES: return t.shape.lanes;
+    case DD_INFO_L: return t.L;
+    case DD_INFO_SMEM_BYTES: return t.smem_bytes;
+    case DD_INFO_GRID: return static_cast<int64_t>(t.ndb) * t.ntj;
+    case DD_INFO_THREADS: return t.shape.threads();
+    case DD_INFO_WORKSPACE_BYTES: return plan->workspace_bytes;
+    case DD_INFO_STAGE_BYTES: return t.stage_bytes_total;
+    case DD_INFO_LAUNCHES: return 2;
+    case DD_INFO_CH: return t.shape.CH;
+    case DD_INFO_NSTAGE: return t.nstage;
+    default: return -1;
+    }
+}
+
+void dd_plan_destroy(dd_plan *plan)
+{
+    if (!plan) return;
+    free_device(plan);
+    delete plan;
+}
+
+const char *dd_strerror(int status)
+{
+    switch (status) {
+    case DD_OK: return "ok";
+    case DD_ERR_INVALID_ARG: return "invalid argument";
+    case DD_ERR_SHIFT_TOO_LARGE: return "largest shift is not smaller than nsamps";
+    case DD_ERR_OVERFLOW: return "channel sum does not fit uint32";
+    case DD_ERR_ALLOC: return "allocation failed";
+    case DD_ERR_CUDA: return "CUDA runtime error";
+    case DD_ERR_UNSUPPORTED_DEVICE: return "current device is not sm_100";
+    case DD_ERR_UNSUPPORTED_PLAN: return "staged window of one DM trial exceeds shared memory";
+    default: return "unknown status";
+    }
+}
+
+const char *dd_version(void) { return "dd 0.1 sm_100a"; }
+
+}  // extern "C"

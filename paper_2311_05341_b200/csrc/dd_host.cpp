@@ -1,0 +1,140 @@
+// dd_host.cpp -- host-only part of libdd.so: the delay table and the
+// plan-time tiling metadata (a2).  No CUDA calls here; compiled with -ffp-contract=off.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <limits>
+
+#include "dd_internal.h"
+
+namespace dd {
+
+namespace {
+// Dispersion constant, MHz^2 s pc^-1 cm^3 (BASELINE.json north_star; reading R1).
+constexpr double kDispersionConstant = 4.148808e3;
+
+inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
+}  // namespace
+
+// Eq. 7: one coefficient per channel, scaled by each DM, divided by the
+// sampling time, rounded to the nearest integer with ties to even (nearbyint under the
+// default rounding mode).  Evaluated in double; the order of operations is
+//   coef = C * (1/f_c^2 - 1/f_high^2);  shift = nearbyint(dm * coef / tsamp).
+int build_shift_table(int nchans, double f_high, double chan_bw, double tsamp,
+                      const double *dm_list, int ndm, int32_t *table, int32_t *max_shift)
+{
+    if (!dm_list || !table || nchans <= 0 || ndm <= 0) return DD_ERR_INVALID_ARG;
+    if (!(f_high > 0.0) || !(chan_bw < 0.0) || !(tsamp > 0.0)) return DD_ERR_INVALID_ARG;
+    if (!std::isfinite(f_high) || !std::isfinite(chan_bw) || !std::isfinite(tsamp))
+        return DD_ERR_INVALID_ARG;
+    const double f_lowest = f_high + static_cast<double>(nchans - 1) * chan_bw;
+    if (!(f_lowest > 0.0)) return DD_ERR_INVALID_ARG;
+    for (int d = 0; d < ndm; ++d)
+        if (!std::isfinite(dm_list[d]) || dm_list[d] < 0.0) return DD_ERR_INVALID_ARG;
+
+    std::vector<double> coef(static_cast<size_t>(nchans));
+    const double inv_top = 1.0 / (f_high * f_high);
+    for (int c = 0; c < nchans; ++c) {
+        const double f = f_high + static_cast<double>(c) * chan_bw;
+        const double inv = 1.0 / (f * f);
+        coef[static_cast<size_t>(c)] = kDispersionConstant * (inv - inv_top);
+    }
+    int32_t biggest = 0;
+    for (int d = 0; d < ndm; ++d) {
+        const double dm = dm_list[d];
+        int32_t *row = table + static_cast<size_t>(d) * static_cast<size_t>(nchans);
+        for (int c = 0; c < nchans; ++c) {
+            const double samples = dm * coef[static_cast<size_t>(c)] / tsamp;
+            const double r = std::nearbyint(samples);
+            if (!(r >= 0.0) || r > static_cast<double>(std::numeric_limits<int32_t>::max()))
+                return DD_ERR_SHIFT_TOO_LARGE;
+            const int32_t s = static_cast<int32_t>(r);
+            row[c] = s;
+            biggest = std::max(biggest, s);
+        }
+    }
+    if (max_shift) *max_shift = biggest;
+    return DD_OK;
+}
+
+// Plan-time tiling (the paper's T_bl / T_diff split, Eq. 6, taken from the
+// exact integer table instead of two separately rounded products): per DM block and channel,
+// the first staged word (block base, aligned down to 4 words = 16 B for the bulk copy) and
+// the staged length; per (DM, channel) the byte offset of its first word inside the stage.
+bool build_tiling(const KernelShape &shape, int variant, const int32_t *table, int ndm,
+                  int nchans, int64_t out_len, int32_t max_shift, int64_t smem_limit,
+                  Tiling *t)
+{
+    const int D_DM = shape.D_DM(), D_J = shape.D_J(), CH = shape.CH;
+    t->shape = shape;
+    t->variant = variant;
+    t->L = round_up((out_len + shape.lanes - 1) / shape.lanes, 16);
+    t->ntj = static_cast<int>((t->L + D_J - 1) / D_J);
+    t->ndb = (ndm + D_DM - 1) / D_DM;
+    t->nch_pad = static_cast<int>(round_up(nchans, CH));
+    t->nk = t->nch_pad / CH;
+    t->Lw = round_up(static_cast<int64_t>(t->ntj) * D_J + max_shift + 4, 4);
+
+    const size_t nbc = static_cast<size_t>(t->ndb) * static_cast<size_t>(t->nch_pad);
+    t->blk_base.assign(nbc, 0);
+    t->blk_len.assign(nbc, D_J * 4);
+    int pitch_words = D_J;
+    int64_t per_jtile_bytes = 0;
+    for (int b = 0; b < t->ndb; ++b) {
+        const int d0 = b * D_DM, d1 = std::min(ndm, d0 + D_DM);
+        for (int c = 0; c < t->nch_pad; ++c) {
+            const size_t i = static_cast<size_t>(b) * t->nch_pad + c;
+            if (c >= nchans) {  // padding channel: a zero row of X, read at offset 0
+                per_jtile_bytes += t->blk_len[i];
+                continue;
+            }
+            int32_t lo = std::numeric_limits<int32_t>::max(), hi = 0;
+            for (int d = d0; d < d1; ++d) {
+                const int32_t s = table[static_cast<size_t>(d) * nchans + c];
+                lo = std::min(lo, s);
+                hi = std::max(hi, s);
+            }
+            const int32_t base = lo & ~3;
+            const int words = static_cast<int>(round_up(static_cast<int64_t>(D_J) + (hi - base), 4));
+            t->blk_base[i] = base;
+            t->blk_len[i] = words * 4;
+            pitch_words = std::max(pitch_words, words);
+            per_jtile_bytes += t->blk_len[i];
+        }
+    }
+    t->pitch_words = pitch_words;
+    const int64_t ofs_stage_bytes = static_cast<int64_t>(D_DM) * CH * 4;
+    const int64_t stage_bytes = static_cast<int64_t>(CH) * pitch_words * 4 + ofs_stage_bytes;
+    const int64_t barrier_bytes = 1024;  // mbarriers + slack, see dd_kernels.cu
+    int nstage = static_cast<int>((smem_limit - barrier_bytes) / stage_bytes);
+    nstage = std::min(nstage, std::min(8, std::max(t->nk, 2)));
+    if (nstage < 2) return false;
+    t->nstage = nstage;
+    t->smem_bytes = barrier_bytes + nstage * stage_bytes;
+    t->stage_bytes_total =
+        (per_jtile_bytes + static_cast<int64_t>(t->ndb) * t->nk * ofs_stage_bytes) * t->ntj;
+
+    // ofs[b][k][dl][cl] = cl*pitch_bytes + 4*(s(d,c) - base(b,c)); DM rows past the end of the
+    // plan repeat the block's last valid row (their results are computed and not stored).
+    t->ofs.assign(static_cast<size_t>(t->ndb) * t->nk * D_DM * CH, 0);
+    const int pitch_bytes = pitch_words * 4;
+    for (int b = 0; b < t->ndb; ++b)
+        for (int k = 0; k < t->nk; ++k)
+            for (int dl = 0; dl < D_DM; ++dl) {
+                const int d = std::min(ndm - 1, b * D_DM + dl);
+                int32_t *dst = t->ofs.data() +
+                               ((static_cast<size_t>(b) * t->nk + k) * D_DM + dl) * CH;
+                for (int cl = 0; cl < CH; ++cl) {
+                    const int c = k * CH + cl;
+                    int32_t o = cl * pitch_bytes;
+                    if (c < nchans) {
+                        const size_t i = static_cast<size_t>(b) * t->nch_pad + c;
+                        o += 4 * (table[static_cast<size_t>(d) * nchans + c] - t->blk_base[i]);
+                    }
+                    dst[cl] = o;
+                }
+            }
+    return true;
+}
+
+}  // namespace dd

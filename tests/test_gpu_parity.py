@@ -1,0 +1,281 @@
+"""-m gpu: the CUDA path (through the C ABI of libdd.so) against the CPU oracle, element by
+element on the same seeded inputs.  Integer inputs: bit-exact.  float32: |gpu - oracle| <=
+1e-4 * sum_c |in| per output (BASELINE.json north_star), and bit-exact on integer-valued
+floats (every partial sum < 2^24, so any summation order gives the same float)."""
+import numpy as np
+import pytest
+
+from paper_2311_05341_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+F32_RTOL_OF_ABS_SUM = 1e-4
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device; the product has no CPU fallback")
+    from paper_2311_05341_b200 import binding, build
+    build.build()
+    binding.lib()
+    return binding
+
+
+def _torch_in(x):
+    import torch
+    if x.dtype == np.uint16:
+        return torch.from_numpy(x.view(np.int16)).cuda().view(torch.uint16)
+    return torch.from_numpy(x).cuda()
+
+
+def gpu_dedisperse(B, x, f_high, chan_bw, tsamp, dms, stream=None):
+    """Run the library on numpy input x [nchans, nsamps]; returns (out numpy, plan facts)."""
+    import torch
+    code = {np.dtype(np.uint8): B.DD_U8, np.dtype(np.uint16): B.DD_U16, np.dtype(np.float32): B.DD_F32}[x.dtype]
+    plan = B.Plan(x.shape[0], x.shape[1], f_high, chan_bw, tsamp, dms, code)
+    try:
+        d_in = _torch_in(np.ascontiguousarray(x))
+        odt = torch.float32 if code == B.DD_F32 else torch.int32
+        d_out = torch.full((plan.ndm, plan.out_len), -7, dtype=odt, device="cuda")
+        plan.execute(d_in, d_out, stream)
+        torch.cuda.synchronize()
+        out = d_out.cpu().numpy()
+        if code != B.DD_F32:
+            out = out.view(np.uint32)
+        return out, plan.shift_table(), plan.out_len, plan.max_shift
+    finally:
+        plan.destroy()
+
+
+def check_against_oracle(oracle, x, gpu_out, table, out_len):
+    if x.dtype == np.float32:
+        ref, ab = oracle.dedisperse(x, table, out_len)
+        err = np.abs(gpu_out.astype(np.float64) - ref)
+        tol = F32_RTOL_OF_ABS_SUM * ab
+        assert (err <= tol).all(), "max err %g, worst err/tol %g" % (err.max(), (err / np.maximum(tol, 1e-300)).max())
+        return float(err.max())
+    ref = oracle.dedisperse(x, table, out_len)
+    bad = np.argwhere(ref != gpu_out)
+    assert bad.size == 0, "first mismatches (d,t): %s of %d" % (bad[:5].tolist(), len(bad))
+    return 0.0
+
+
+def _rand_input(rng, dtype, nchans, nsamps):
+    if dtype == np.float32:
+        return rng.standard_normal((nchans, nsamps)).astype(np.float32)
+    hi = 256 if dtype == np.uint8 else 65536
+    return rng.integers(0, hi, (nchans, nsamps)).astype(dtype)
+
+
+# ------------------------------------------------------------------ configs[0]: tiny, full
+def test_tiny_config_bit_exact_and_pulse(B, oracle, golden):
+    cfg = W.CONFIGS["tiny"]
+    otab, omx = oracle.shift_table(cfg.nchans, cfg.f_high, cfg.chan_bw, cfg.tsamp, cfg.dm_list)
+    x = W.make_input_numpy(cfg, otab, cfg.nsamps - omx)
+    out, tab, out_len, mx = gpu_dedisperse(B, x, cfg.f_high, cfg.chan_bw, cfg.tsamp, cfg.dm_list)
+    assert np.array_equal(tab, otab) and mx == omx and out_len == 3966
+    check_against_oracle(oracle, x, out, otab, out_len)
+    # the paper's own check: the injected pulse is recovered at its DM
+    g = golden("tiny_pulse_pins.json")["noisy"]
+    box = out[:, :-3].astype(np.int64) + out[:, 1:-2] + out[:, 2:-1] + out[:, 3:]
+    d, t = np.unravel_index(np.argmax(box), box.shape)
+    assert (d, t) == (17, g["boxcar4_dm17_t"]) and box[d, t] == g["boxcar4_dm17"]
+    assert out[17, 1000] == g["value_dm17_t1000"]
+
+
+def test_tiny_noise_free_pulse_profile(B, oracle, golden):
+    cfg = W.CONFIGS["tiny"]
+    otab, omx = oracle.shift_table(cfg.nchans, cfg.f_high, cfg.chan_bw, cfg.tsamp, cfg.dm_list)
+    x = W.make_input_numpy(cfg, otab, cfg.nsamps - omx, noise=False)
+    out, _, _, _ = gpu_dedisperse(B, x, cfg.f_high, cfg.chan_bw, cfg.tsamp, cfg.dm_list)
+    g = golden("tiny_pulse_pins.json")["noise_free"]
+    peaks = (out.max(axis=1).astype(np.int64) - g["baseline"])[g["dm_lo"]:g["dm_lo"] + 15]
+    assert peaks.tolist() == g["max_minus_baseline"]
+    assert np.flatnonzero(out[17] == g["row17_peak_value"]).tolist() == g["row17_peak_t"]
+
+
+# ------------------------------------------------------------------ closed forms on the GPU
+def test_closed_form_ramp_all_dtypes(B):
+    # in[c][t] = 100c + t => out[d][t] = 600 + 4t + sum_c s(d,c); table rows (0,3,6,10),(0,6,13,20)
+    nsamps = 32
+    ramp = 100 * np.arange(4)[:, None] + np.arange(nsamps)[None, :]
+    for dt in (np.uint16, np.float32):
+        out, tab, out_len, mx = gpu_dedisperse(B, ramp.astype(dt), 1500.0, -25.0, 1e-3, [0.0, 50.0, 100.0])
+        assert mx == 20 and out_len == 12
+        t = np.arange(12)
+        for d, k in enumerate((600, 619, 639)):
+            assert out[d].tolist() == (k + 4 * t).tolist()
+    small = (10 * np.arange(4)[:, None] + np.arange(nsamps)[None, :]).astype(np.uint8)
+    out, _, _, _ = gpu_dedisperse(B, small, 1500.0, -25.0, 1e-3, [0.0, 50.0, 100.0])
+    for d, k in enumerate((60, 79, 99)):
+        assert out[d].tolist() == (k + 4 * np.arange(12)).tolist()
+
+
+@pytest.mark.parametrize("nchans", [256, 257, 258, 520, 1031])
+def test_u8_packed_lane_flush_all_255(B, nchans):
+    # a 16-bit lane holds at most 257 samples of 255: the flush must come in time
+    x = np.full((nchans, 700), 255, dtype=np.uint8)
+    out, _, _, _ = gpu_dedisperse(B, x, 1500.0, -300.0 / nchans, 64e-6, [0.0, 3.0, 40.0])
+    assert (out == 255 * nchans).all()
+
+
+def test_u16_all_max(B):
+    nchans = 600
+    x = np.full((nchans, 900), 65535, dtype=np.uint16)
+    out, _, _, _ = gpu_dedisperse(B, x, 400.0, -0.05, 1e-4, [0.0, 1.0, 2.5])
+    assert (out == 65535 * nchans).all()
+
+
+def test_f32_all_ones(B):
+    x = np.ones((300, 1500), dtype=np.float32)
+    out, _, _, _ = gpu_dedisperse(B, x, 1500.0, -1.0, 64e-6, [0.0, 10.0, 20.0])
+    assert (out == 300.0).all()
+
+
+# ------------------------------------------------------------------ random plans, ragged everything
+CASES = [
+    # nchans, nsamps, ndm, dm_step, f_high, band, tsamp   (several tiles + ragged tails)
+    (37, 5003, 19, 3.0, 1500.0, 300.0, 64e-6),
+    (64, 9001, 33, 1.0, 1550.0, 400.0, 64e-6),
+    (130, 4100, 70, 0.5, 400.0, 100.0, 256e-6),
+    (16, 70001, 5, 11.0, 1400.0, 200.0, 32e-6),
+    (300, 3000, 17, 0.1, 190.0, 60.0, 655.36e-6),
+]
+
+
+@pytest.mark.parametrize("dtype", [np.uint8, np.uint16, np.float32])
+@pytest.mark.parametrize("case", CASES)
+def test_random_plans_match_oracle(B, oracle, dtype, case):
+    nchans, nsamps, ndm, step, f_high, band, tsamp = case
+    rng = np.random.default_rng([nchans, nsamps, ndm])
+    x = _rand_input(rng, dtype, nchans, nsamps)
+    dms = np.arange(ndm) * step
+    out, tab, out_len, mx = gpu_dedisperse(B, x, f_high, -band / nchans, tsamp, dms)
+    otab, omx = oracle.shift_table(nchans, f_high, -band / nchans, tsamp, dms)
+    assert np.array_equal(tab, otab) and mx == omx and out_len == nsamps - omx
+    check_against_oracle(oracle, x, out, otab, out_len)
+
+
+def test_f32_integer_valued_is_bit_exact(B, oracle):
+    # pins the f32 kernel's indexing as tightly as the integer paths
+    rng = np.random.default_rng(11)
+    x = rng.integers(0, 256, (200, 6000)).astype(np.float32)
+    dms = np.arange(40) * 2.0
+    out, tab, out_len, _ = gpu_dedisperse(B, x, 1500.0, -1.5, 64e-6, dms)
+    ref, _ = oracle.dedisperse(x, tab, out_len)
+    assert np.array_equal(out.astype(np.float64), ref)
+
+
+# ------------------------------------------------------------------ degenerate cases
+@pytest.mark.parametrize("dtype", [np.uint8, np.uint16, np.float32])
+def test_single_dm_single_channel(B, oracle, dtype):
+    rng = np.random.default_rng(3)
+    x = _rand_input(rng, dtype, 1, 100)
+    out, tab, out_len, mx = gpu_dedisperse(B, x, 1500.0, -1.0, 1e-3, [5.0])
+    assert mx == 0 and out_len == 100 and tab.tolist() == [[0]]
+    assert np.array_equal(out[0], x[0].astype(out.dtype))
+
+
+@pytest.mark.parametrize("dtype", [np.uint8, np.uint16, np.float32])
+def test_out_len_one(B, oracle, dtype):
+    # max_shift = nsamps - 1: one output sample per DM
+    rng = np.random.default_rng(4)
+    tab, mx = B.dd_shift_table_build(4, 1500.0, -25.0, 1e-3, [0.0, 50.0, 100.0])
+    x = _rand_input(rng, dtype, 4, mx + 1)
+    if dtype == np.float32:
+        x = np.rint(x * 8).astype(np.float32)
+    out, tab2, out_len, _ = gpu_dedisperse(B, x, 1500.0, -25.0, 1e-3, [0.0, 50.0, 100.0])
+    assert out_len == 1 and np.array_equal(tab, tab2)
+    for d in range(3):
+        assert float(out[d, 0]) == float(sum(float(x[c, tab[d, c]]) for c in range(4)))
+
+
+def test_unsorted_and_repeated_dm_list(B, oracle):
+    rng = np.random.default_rng(5)
+    x = _rand_input(rng, np.uint8, 48, 4000)
+    dms = np.array([30.0, 0.0, 12.5, 30.0, 7.0, 99.0, 1.0, 55.5, 0.0, 80.0] * 4)
+    out, tab, out_len, _ = gpu_dedisperse(B, x, 1400.0, -2.0, 64e-6, dms)
+    otab, _ = oracle.shift_table(48, 1400.0, -2.0, 64e-6, dms)
+    assert np.array_equal(tab, otab)
+    check_against_oracle(oracle, x, out, otab, out_len)
+
+
+def test_single_impulse_response(B):
+    # a single 1 at (c*, tau) in zeros -> out[d][tau - s(d,c*)] = 1 and 0 elsewhere
+    nchans, nsamps, cstar, tau = 40, 3000, 29, 1777
+    x = np.zeros((nchans, nsamps), dtype=np.uint16)
+    x[cstar, tau] = 1
+    dms = np.arange(24) * 4.0
+    out, tab, out_len, _ = gpu_dedisperse(B, x, 1500.0, -5.0, 64e-6, dms)
+    expect = np.zeros_like(out)
+    for d in range(len(dms)):
+        t = tau - tab[d, cstar]
+        if 0 <= t < out_len:
+            expect[d, t] = 1
+    assert np.array_equal(out, expect)
+
+
+@pytest.mark.parametrize("dtype", [np.uint8, np.uint16, np.float32])
+def test_misaligned_input_pointer_and_odd_row_length(B, oracle, dtype):
+    # rows that are not 4/8/16-byte aligned take the scalar path of the pre-pass
+    import torch
+    rng = np.random.default_rng(6)
+    nchans, nsamps = 21, 2999
+    x = _rand_input(rng, dtype, nchans, nsamps)
+    if dtype == np.float32:
+        x = np.rint(x * 16).astype(np.float32)
+    dms = np.arange(9) * 7.0
+    code = {np.uint8: B.DD_U8, np.uint16: B.DD_U16, np.float32: B.DD_F32}[dtype]
+    plan = B.Plan(nchans, nsamps, 1500.0, -10.0, 64e-6, dms, code)
+    flat = _torch_in(np.concatenate([np.zeros(1, dtype=dtype), x.ravel()]))
+    d_in = flat[1:]  # element-misaligned view
+    assert d_in.data_ptr() % 16 != 0
+    odt = torch.float32 if code == B.DD_F32 else torch.int32
+    d_out = torch.empty((plan.ndm, plan.out_len), dtype=odt, device="cuda")
+    plan.execute(d_in.data_ptr(), d_out)
+    torch.cuda.synchronize()
+    out = d_out.cpu().numpy()
+    out = out if code == B.DD_F32 else out.view(np.uint32)
+    check_against_oracle(oracle, x, out, plan.shift_table(), plan.out_len)
+    plan.destroy()
+
+
+def test_repeat_execute_streams_and_host_path(B, oracle):
+    import torch
+    rng = np.random.default_rng(8)
+    nchans, nsamps = 96, 20000
+    dms = np.arange(50) * 3.0
+    plan = B.Plan(nchans, nsamps, 1500.0, -3.0, 64e-6, dms, B.DD_U8)
+    ref = None
+    st = torch.cuda.Stream()
+    for it in range(3):
+        x = _rand_input(rng, np.uint8, nchans, nsamps)
+        d_in = _torch_in(x)
+        d_out = torch.empty((plan.ndm, plan.out_len), dtype=torch.int32, device="cuda")
+        torch.cuda.synchronize()
+        with torch.cuda.stream(st):
+            plan.execute(d_in, d_out)  # picks up the current (side) stream
+        st.synchronize()
+        out = d_out.cpu().numpy().view(np.uint32)
+        ref = oracle.dedisperse(x, plan.shift_table(), plan.out_len)
+        assert np.array_equal(out, ref)
+    # dd_execute_host on the last input
+    h_in = torch.from_numpy(x).pin_memory()
+    h_out = torch.empty((plan.ndm, plan.out_len), dtype=torch.int32).pin_memory()
+    plan.execute_host(h_in, h_out)
+    assert np.array_equal(h_out.numpy().view(np.uint32), ref)
+    plan.destroy()
+
+
+def test_plan_errors_on_gpu(B):
+    with pytest.raises(B.DDError) as e:
+        B.Plan(4, 32, 1500.0, -25.0, 1e-3, [0.0, 300.0], B.DD_U8)
+    assert e.value.status == B.DD_ERR_SHIFT_TOO_LARGE
+    plan = B.Plan(4, 32, 1500.0, -25.0, 1e-3, [0.0], B.DD_U8)
+    with pytest.raises(B.DDError) as e:
+        plan.execute(0, 0)
+    assert e.value.status == B.DD_ERR_INVALID_ARG
+    plan.destroy()
+    plan.destroy()  # idempotent
