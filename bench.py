@@ -1,0 +1,351 @@
+#!/usr/bin/env python
+"""bench.py -- dedispersion adds/s on synthetic filterbank data (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config NAME] [--impl reference]
+
+One "step" = one pass of the whole hot path (dd_execute: lane-interleave pre-pass + the
+dedispersion kernel) over one block of synthetic input of the named config.  Default
+workload: `headline` (BASELINE.json configs[3], 8192 channels x 2^18 samples uint8, 1024 DM
+trials -- the config north_star's target is quoted on; it fits one GPU).  Prints ONE JSON line.
+
+N > 1 (launched by torch.distributed.run): every rank processes its own block of the same
+shape (independent time shards of a longer observation); no data-path
+collective; value = units of all ranks / max-over-ranks time ("scaling": "weak").
+
+--impl reference: the CPU oracle (oracle/dedisp_oracle.c), as it stands, timed on the host
+cores on a bounded sample of the same workload (a subset of DM rows per step).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2311_05341_b200 import workloads as W  # noqa: E402
+
+METRIC = "dedispersion adds/s (DM*sample*channel per s)"
+UNIT = "adds/s"
+N_SM = 148
+# Plain integer ALU peak: 64 INT32 add lanes per SM per clock (alu
+# pipe: 4 sub-partitions x 16 lanes, B300_MICROARCH.md "Pipe rates") x 148 SMs x max SM clock.
+INT_LANES_PER_SM_CLK = 64
+# Shared-memory bandwidth (paper's Eq. 8): 32 banks x 4 B per SM per clock.
+SMEM_BYTES_PER_SM_CLK = 128
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return float(p["hbm_gbs"]), float(p.get("sm_max_mhz", 1965.0)), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t0: float, t1: float):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ts, line in self.rows:
+            if not (t0 <= ts <= t1 + 0.12):
+                continue
+            f = [x.strip() for x in line.split(",")]
+            try:
+                sm.append(float(f[0]))
+                mx = float(f[1])
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def _dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+# ------------------------------------------------------------------------- reference arm
+def _oracle_sample(cfg, oracle, rows_per_step: int):
+    """A bounded sample of the workload for the CPU oracle: the full-shape input, a subset of
+    DM rows spread over the plan (adds/s of the triple loop does not depend on which rows)."""
+    table, mx = oracle.shift_table(cfg.nchans, cfg.f_high, cfg.chan_bw, cfg.tsamp, cfg.dm_list)
+    out_len = cfg.nsamps - mx
+    rows = np.unique(np.linspace(0, cfg.ndm - 1, rows_per_step).astype(np.int64))
+    return table[rows], out_len, len(rows)
+
+
+def _host_input(cfg):
+    # same distribution as the device generator; values do not matter for CPU timing
+    rng = np.random.default_rng(cfg.seed)
+    if cfg.in_dtype == W.F32:
+        return rng.standard_normal((cfg.nchans, cfg.nsamps), dtype=np.float32)
+    hi = 255 if cfg.in_dtype == W.U8 else 65535
+    x = np.empty((cfg.nchans, cfg.nsamps), dtype=cfg.np_dtype)
+    step = max(1, (1 << 24) // cfg.nsamps)
+    for c0 in range(0, cfg.nchans, step):
+        blk = rng.standard_normal((min(step, cfg.nchans - c0), cfg.nsamps), dtype=np.float32)
+        x[c0:c0 + step] = np.clip(np.rint(blk * cfg.sd + cfg.mean), 0, hi).astype(cfg.np_dtype)
+    return x
+
+
+def time_oracle(cfg, steps: int, warmup: int, rows_per_step: int | None = None, x=None):
+    from oracle import oracle
+    oracle.build()
+    threads = oracle.omp_threads()
+    if rows_per_step is None:
+        rows_per_step = max(threads, 4)
+    sub, out_len, nrows = _oracle_sample(cfg, oracle, rows_per_step)
+    if x is None:
+        x = _host_input(cfg)
+    for _ in range(warmup):
+        oracle.dedisperse(x, sub[:max(1, min(nrows, threads))], out_len)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        oracle.dedisperse(x, sub, out_len)
+    dt = time.perf_counter() - t0
+    adds = float(nrows) * out_len * cfg.nchans * steps
+    return {"value": adds / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": "%d of %d DM rows x full out_len x all %d channels per step, %d step(s), %.1f s"
+                      % (nrows, cfg.ndm, cfg.nchans, steps, dt)}, dt / steps
+
+
+def run_reference(args):
+    rank, _, world = _dist_env()
+    if rank != 0:
+        return 0
+    cfg = W.CONFIGS[args.config]
+    base, ms = time_oracle(cfg, args.steps, args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": base["value"], "unit": UNIT,
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": _dtype_name(cfg), "data": "synthetic",
+            "config": _config_dict(cfg, None), "cpu_baseline": base,
+            "e2e": {"value": base["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def _dtype_name(cfg):
+    return {W.U8: "u8 in, packed u16/u32 integer accumulate, u32 out",
+            W.U16: "u16 in, u32 integer accumulate, u32 out",
+            W.F32: "f32"}[cfg.in_dtype]
+
+
+def _config_dict(cfg, plan):
+    d = {"workload": cfg.name, "nchans": cfg.nchans, "nsamps": cfg.nsamps, "ndm": cfg.ndm,
+         "dm_step": cfg.dm_step, "f_high_MHz": cfg.f_high, "chan_bw_MHz": cfg.chan_bw,
+         "tsamp_s": cfg.tsamp, "in_dtype": W.DTYPE_NAME[cfg.in_dtype],
+         "l2": "input (%.2f GiB) and output are each larger than the 126 MB L2; no flush needed"
+               % (cfg.nchans * cfg.nsamps * W.ELEM_BYTES[cfg.in_dtype] / 2 ** 30)}
+    if plan is not None:
+        d.update({"out_len": plan.out_len, "max_shift": plan.max_shift,
+                  "adds_per_step": plan.ndm * plan.out_len * cfg.nchans,
+                  "adds_nominal": cfg.ndm * cfg.nsamps * cfg.nchans,
+                  "tile": "D_DM=%d x D_J=%d words x %d lanes, CH=%d, %d stages, %d B smem, grid %d x %d threads"
+                          % (plan.info("D_DM"), plan.info("D_J"), plan.info("LANES"), plan.info("CH"),
+                             plan.info("NSTAGE"), plan.info("SMEM_BYTES"), plan.info("GRID"),
+                             plan.info("THREADS"))})
+    return d
+
+
+# ------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import torch
+    rank, local_rank, world = _dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    from paper_2311_05341_b200 import binding as B, build
+    if rank == 0:
+        build.build()
+    if dist is not None:
+        dist.barrier()
+    B.lib()
+
+    cfg = W.CONFIGS[args.config]
+    hbm_gbs, sm_max_mhz, peak_kind = _peaks()
+    plan = B.Plan(cfg.nchans, cfg.nsamps, cfg.f_high, cfg.chan_bw, cfg.tsamp, cfg.dm_list, cfg.in_dtype)
+    table = plan.shift_table() if cfg.npulses else None
+    # every rank: its own block (seed offset by rank), resident in HBM before timing starts
+    import dataclasses
+    x = W.make_input_torch(dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank), "cuda", table, plan.out_len)
+    odt = torch.float32 if cfg.in_dtype == W.F32 else torch.int32
+    out = torch.empty((plan.ndm, plan.out_len), dtype=odt, device="cuda")
+    adds = plan.ndm * plan.out_len * cfg.nchans
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing
+    for _ in range(args.warmup):
+        plan.execute(x, out)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    plan.set_timing(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t_host0 = time.perf_counter()
+    e0.record(stream)
+    for _ in range(args.steps):
+        plan.execute(x, out)
+    e1.record(stream)
+    barrier()
+    t_host1 = time.perf_counter()
+    ms_total = e0.elapsed_time(e1)
+    plan.set_timing(False)
+    il_ms, main_ms = plan.kernel_times(min(64, args.steps))
+    clocks = sampler.stop(t_host0, t_host1) if rank == 0 else None
+    if dist is not None:
+        t = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * adds / (ms_step * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers (H2D + kernels + D2H in the timed region)
+    h_in = torch.empty(x.shape, dtype=x.dtype).pin_memory()
+    h_in.copy_(x)
+    h_out = torch.empty(out.shape, dtype=out.dtype).pin_memory()
+    e2e_steps = max(1, min(args.steps, 5))
+    plan.execute_host(h_in, h_out)  # warm-up (allocates the plan's device buffers)
+    barrier()
+    e0.record(stream)
+    for _ in range(e2e_steps):
+        plan.execute_host(h_in, h_out)
+    e1.record(stream)
+    barrier()
+    ms_e2e = e0.elapsed_time(e1)
+    if dist is not None:
+        t = torch.tensor([ms_e2e], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_e2e = float(t.item())
+    ms_e2e /= e2e_steps
+    h2d = h_in.numel() * h_in.element_size()
+    d2h = h_out.numel() * h_out.element_size()
+    checksum = int(h_out.view(torch.int32)[:, ::4097].to(torch.int64).sum().item())
+
+    if rank != 0:
+        plan.destroy()
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
+        return 0
+
+    # ---- rooflines of the dominant kernel (dedisperse_kernel), from its own CUDA events
+    main_s = float(np.mean(main_ms)) * 1e-3
+    il_s = float(np.mean(il_ms)) * 1e-3
+    kadds = adds / main_s
+    clk = sm_max_mhz * 1e6
+    int_peak = N_SM * INT_LANES_PER_SM_CLK * clk
+    smem_peak_gbs = N_SM * SMEM_BYTES_PER_SM_CLK * clk / 1e9
+    in_b = W.ELEM_BYTES[cfg.in_dtype]
+    smem_alg_bytes = adds * in_b                      # one sample read from shared memory per add
+    hbm_alg_bytes = cfg.nchans * cfg.nsamps * in_b + plan.ndm * plan.out_len * 4
+    roofline = {"bound": "alu", "kernel": "dedisperse_kernel",
+                "achieved": kadds / 1e12, "peak": int_peak / 1e12, "unit": "Tadd/s",
+                "frac": kadds / int_peak, "traffic": None,
+                "peak_kind": "derived: %d SMs x %d INT32 add lanes/clk x %.0f MHz (%s sm_max_mhz)"
+                             % (N_SM, INT_LANES_PER_SM_CLK, sm_max_mhz, peak_kind),
+                "note": "achieved counts sample-adds; one packed IADD3 lane-instruction performs up "
+                        "to 4 (u8) / 2 (u16) sample-adds, so frac may exceed 1",
+                "kernel_ms": main_s * 1e3, "share_of_step": main_s / (main_s + il_s)}
+    roofline_smem = {"bound": "smem", "achieved": smem_alg_bytes / main_s / 1e9, "peak": smem_peak_gbs,
+                     "unit": "GB/s", "frac": smem_alg_bytes / main_s / 1e9 / smem_peak_gbs,
+                     "peak_kind": "derived (paper Eq. 8): %d SMs x %d B/clk x %.0f MHz"
+                                  % (N_SM, SMEM_BYTES_PER_SM_CLK, sm_max_mhz),
+                     "bytes_per_add": in_b}
+    roofline_hbm = {"bound": "hbm", "achieved": hbm_alg_bytes / (ms_step * 1e-3) / 1e9, "peak": hbm_gbs,
+                    "unit": "GB/s", "frac": hbm_alg_bytes / (ms_step * 1e-3) / 1e9 / hbm_gbs,
+                    "peak_kind": peak_kind + " copy bandwidth",
+                    "staged_l2_to_smem_bytes": plan.info("STAGE_BYTES")}
+
+    cpu_base, _ = time_oracle(cfg, 1, 1, x=h_in.numpy() if cfg.in_dtype != W.U16
+                              else h_in.view(torch.int16).numpy().view(np.uint16))
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": _dtype_name(cfg),
+            "data": "synthetic", "config": _config_dict(cfg, plan),
+            "realtime_factor": {"t_obs_over_t": cfg.nsamps * cfg.tsamp / (ms_step * 1e-3),
+                                "out_len_tsamp_over_t": plan.out_len * cfg.tsamp / (ms_step * 1e-3)},
+            "value_nominal": world * cfg.ndm * cfg.nsamps * cfg.nchans / (ms_step * 1e-3),
+            "kernels_ms": {"interleave_kernel": il_s * 1e3, "dedisperse_kernel": main_s * 1e3},
+            "roofline": roofline, "roofline_smem": roofline_smem, "roofline_hbm": roofline_hbm,
+            "cpu_baseline": cpu_base,
+            "e2e": {"value": world * adds / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
+                    "steps": e2e_steps, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "api": "dd_execute_host (pinned host buffers)", "checksum": checksum},
+            "gpu_launches": args.steps * plan.info("LAUNCHES"),
+            "clocks": clocks}
+    print(json.dumps(line))
+    plan.destroy()
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="headline", choices=list(W.CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
