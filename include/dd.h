@@ -65,6 +65,9 @@ int dd_shift_table_build(int nchans, double f_high_MHz, double chan_bw_MHz, doub
  * nsamps <= 0, unknown dtype); DD_ERR_SHIFT_TOO_LARGE (max shift >= nsamps);
  * DD_ERR_OVERFLOW (u8: 255*nchans >= 2^32; u16: 65535*nchans >= 2^32); DD_ERR_ALLOC;
  * DD_ERR_CUDA; DD_ERR_UNSUPPORTED_DEVICE; DD_ERR_UNSUPPORTED_PLAN.
+ * Tuning aid: if the environment variable DD_FORCE_VARIANT=<n> is set, entry n of the
+ * compiled kernel table (dd_kernels.cu) is used instead of the automatic choice; the
+ * results are identical, only the tiling differs (A/B measurements under profiles/).
  */
 int dd_plan_create(dd_plan **out, int nchans, int64_t nsamps, double f_high_MHz,
                    double chan_bw_MHz, double tsamp_s, const double *dm_list, int ndm,
@@ -107,9 +110,9 @@ int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_str
  */
 enum {
     DD_INFO_D_DM = 0,          /* DM trials per thread block */
-    DD_INFO_D_J = 1,           /* 32-bit words of the interleaved time axis per thread block */
-    DD_INFO_LANES = 2,         /* samples per 32-bit word: 4 (u8), 2 (u16), 1 (f32) */
-    DD_INFO_L = 3,             /* lane stride L: word j, lane k holds in[c][k*L + j] */
+    DD_INFO_D_J = 1,           /* superwords of the interleaved time axis per thread block */
+    DD_INFO_LANES = 2,         /* samples per superword (4, 8 or 16 bytes of one channel) */
+    DD_INFO_L = 3,             /* lane stride L: superword j, lane k holds in[c][k*L + j] */
     DD_INFO_SMEM_BYTES = 4,    /* dynamic shared memory per thread block */
     DD_INFO_GRID = 5,          /* thread blocks of the main kernel */
     DD_INFO_THREADS = 6,       /* threads per block of the main kernel */

@@ -19,7 +19,8 @@ struct dd_plan {
     dd::Tiling til;
     // device
     uint32_t *d_X = nullptr;
-    int32_t *d_ofs = nullptr, *d_base = nullptr, *d_len = nullptr;
+    uint8_t *d_ofs = nullptr;
+    int32_t *d_blk = nullptr;
     int64_t workspace_bytes = 0;
     // dd_execute_host buffers (lazy)
     void *d_in_own = nullptr, *d_out_own = nullptr;
@@ -44,8 +45,7 @@ void free_device(dd_plan *p)
         cudaDeviceSynchronize();
         cudaFree(p->d_X);
         cudaFree(p->d_ofs);
-        cudaFree(p->d_base);
-        cudaFree(p->d_len);
+        cudaFree(p->d_blk);
         cudaFree(p->d_in_own);
         cudaFree(p->d_out_own);
         if (p->ev_made)
@@ -130,9 +130,12 @@ int dd_plan_create(dd_plan **out, int nchans, int64_t nsamps, double f_high_MHz,
 
         // first compiled variant of this dtype whose shared-memory ring fits
         bool found = false;
+        const char *force = std::getenv("DD_FORCE_VARIANT");  // tuning experiments only
+        const int forced = force ? std::atoi(force) : -1;
         for (int v = 0; v < dd::num_variants() && !found; ++v) {
             const dd::KernelShape &sh = dd::variant_shape(v);
             if (sh.mode != in_dtype) continue;
+            if (forced >= 0 ? v != forced : sh.tune != 0) continue;
             found = dd::build_tiling(sh, v, p->table.data(), ndm, nchans, p->out_len, p->max_shift,
                                      smem_limit, &p->til);
         }
@@ -143,7 +146,7 @@ int dd_plan_create(dd_plan **out, int nchans, int64_t nsamps, double f_high_MHz,
         }
         const dd::Tiling &t = p->til;
         if (dd::variant_prepare(t.variant, static_cast<int>(t.smem_bytes)) != 0) rc = DD_ERR_CUDA;
-        const size_t xbytes = static_cast<size_t>(t.nch_pad) * t.Lw * 4;
+        const size_t xbytes = static_cast<size_t>(t.nch_pad) * t.Lw * t.shape.sw_bytes();
         if (rc == DD_OK && cudaMalloc(reinterpret_cast<void **>(&p->d_X), xbytes) != cudaSuccess) {
             cudaGetLastError();
             rc = DD_ERR_ALLOC;
@@ -151,15 +154,13 @@ int dd_plan_create(dd_plan **out, int nchans, int64_t nsamps, double f_high_MHz,
         // padding channel rows stay zero for the life of the plan
         if (rc == DD_OK && cudaMemset(p->d_X, 0, xbytes) != cudaSuccess) rc = DD_ERR_CUDA;
         if (rc == DD_OK) rc = upload(&p->d_ofs, t.ofs);
-        if (rc == DD_OK) rc = upload(&p->d_base, t.blk_base);
-        if (rc == DD_OK) rc = upload(&p->d_len, t.blk_len);
+        if (rc == DD_OK) rc = upload(&p->d_blk, t.blk);
         if (rc == DD_OK && cudaDeviceSynchronize() != cudaSuccess) rc = DD_ERR_CUDA;
         p->workspace_bytes = static_cast<int64_t>(xbytes) +
-                             static_cast<int64_t>((t.ofs.size() + t.blk_base.size() + t.blk_len.size()) * 4);
+                             static_cast<int64_t>(t.ofs.size() + t.blk.size() * 4);
         // the host copies of the tiling tables are no longer needed
-        std::vector<int32_t>().swap(p->til.ofs);
-        std::vector<int32_t>().swap(p->til.blk_base);
-        std::vector<int32_t>().swap(p->til.blk_len);
+        std::vector<uint8_t>().swap(p->til.ofs);
+        std::vector<int32_t>().swap(p->til.blk);
     } catch (const std::bad_alloc &) {
         rc = DD_ERR_ALLOC;
     }
@@ -198,14 +199,13 @@ int dd_execute(const dd_plan *plan, const void *d_in, void *d_out, void *cuda_st
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const cudaEvent_t *ev = plan->timing ? plan->ev[plan->timed_count % dd_plan::kRing] : nullptr;
     if (ev) cudaEventRecord(ev[0], st);
-    if (dd::launch_interleave(plan->in_dtype, ip, cuda_stream) != 0) return DD_ERR_CUDA;
+    if (dd::launch_interleave(plan->in_dtype, t.shape.VW, ip, cuda_stream) != 0) return DD_ERR_CUDA;
     if (ev) cudaEventRecord(ev[1], st);
 
     dd::KernelParams kp;
     kp.X = plan->d_X;
     kp.ofs = plan->d_ofs;
-    kp.blk_base = plan->d_base;
-    kp.blk_len = plan->d_len;
+    kp.blk = plan->d_blk;
     kp.out = d_out;
     kp.out_len = plan->out_len;
     kp.Lw = t.Lw;
@@ -215,9 +215,10 @@ int dd_execute(const dd_plan *plan, const void *d_in, void *d_out, void *cuda_st
     kp.nk = t.nk;
     kp.ndb = t.ndb;
     kp.ntj = t.ntj;
-    kp.pitch_bytes = t.pitch_words * 4;
+    kp.rows_bytes = t.rows_bytes;
     kp.nstage = t.nstage;
-    kp.stage_bytes = t.shape.CH * t.pitch_words * 4 + t.shape.D_DM() * t.shape.CH * 4;
+    kp.stage_bytes = t.rows_bytes + t.shape.D_DM() * t.shape.CH * t.shape.OW;
+    kp.one = 1u;
     const int grid = t.ndb * t.ntj;
     if (dd::launch_dedisperse(t.variant, kp, grid, static_cast<int>(t.smem_bytes), cuda_stream) != 0)
         return DD_ERR_CUDA;
@@ -294,7 +295,7 @@ int64_t dd_plan_info(const dd_plan *plan, int what)
     switch (what) {
     case DD_INFO_D_DM: return t.shape.D_DM();
     case DD_INFO_D_J: return t.shape.D_J();
-    case DD_INFO_LANES: return t.shape.lanes;
+    case DD_INFO_LANES: return t.shape.lanes();
     case DD_INFO_L: return t.L;
     case DD_INFO_SMEM_BYTES: return t.smem_bytes;
     case DD_INFO_GRID: return static_cast<int64_t>(t.ndb) * t.ntj;

@@ -59,54 +59,80 @@ int build_shift_table(int nchans, double f_high, double chan_bw, double tsamp,
 
 // Plan-time tiling (the paper's T_bl / T_diff split, Eq. 6, taken from the
 // exact integer table instead of two separately rounded products): per DM block and channel,
-// the first staged word (block base, aligned down to 4 words = 16 B for the bulk copy) and
-// the staged length; per (DM, channel) the byte offset of its first word inside the stage.
+// the first staged superword (block base, aligned down to a 16-byte address for the bulk
+// copy) and the staged length; per (DM, channel) the byte offset of its first superword
+// inside the stage buffer.  Windows are packed back to back in a stage.
 bool build_tiling(const KernelShape &shape, int variant, const int32_t *table, int ndm,
                   int nchans, int64_t out_len, int32_t max_shift, int64_t smem_limit,
                   Tiling *t)
 {
     const int D_DM = shape.D_DM(), D_J = shape.D_J(), CH = shape.CH;
+    const int S = shape.sw_bytes();  // bytes per superword
+    const int A = 16 / S;            // superwords per 16 bytes (bulk-copy granule)
     t->shape = shape;
     t->variant = variant;
-    t->L = round_up((out_len + shape.lanes - 1) / shape.lanes, 16);
+    t->L = round_up((out_len + shape.lanes() - 1) / shape.lanes(), 16);
     t->ntj = static_cast<int>((t->L + D_J - 1) / D_J);
     t->ndb = (ndm + D_DM - 1) / D_DM;
     t->nch_pad = static_cast<int>(round_up(nchans, CH));
     t->nk = t->nch_pad / CH;
     t->Lw = round_up(static_cast<int64_t>(t->ntj) * D_J + max_shift + 4, 4);
 
-    const size_t nbc = static_cast<size_t>(t->ndb) * static_cast<size_t>(t->nch_pad);
-    t->blk_base.assign(nbc, 0);
-    t->blk_len.assign(nbc, D_J * 4);
-    int pitch_words = D_J;
+    // Channel permutation: slot i of the first half of each stage takes channels from the
+    // top of the band (short windows), the second half mirrors them from the bottom (long
+    // windows; padding channels c >= nchans count as the bottom).  Window length grows
+    // almost linearly with the channel index, so every stage gets about the same bytes.
+    t->chan.assign(static_cast<size_t>(t->nch_pad), 0);
+    for (int k = 0; k < t->nk; ++k)
+        for (int cl = 0; cl < CH; ++cl) {
+            const int h = CH / 2;
+            t->chan[static_cast<size_t>(k) * CH + cl] =
+                cl < h ? k * h + cl : t->nch_pad - 1 - (k * h + (cl - h));
+        }
+
+    const size_t nslot = static_cast<size_t>(t->ndb) * static_cast<size_t>(t->nch_pad);
+    t->blk.assign(nslot * 4, 0);
+    int rows_bytes = 0;
     int64_t per_jtile_bytes = 0;
     for (int b = 0; b < t->ndb; ++b) {
         const int d0 = b * D_DM, d1 = std::min(ndm, d0 + D_DM);
-        for (int c = 0; c < t->nch_pad; ++c) {
-            const size_t i = static_cast<size_t>(b) * t->nch_pad + c;
-            if (c >= nchans) {  // padding channel: a zero row of X, read at offset 0
-                per_jtile_bytes += t->blk_len[i];
-                continue;
+        for (int k = 0; k < t->nk; ++k) {
+            int dst = 0;
+            for (int cl = 0; cl < CH; ++cl) {
+                const size_t slot = static_cast<size_t>(b) * t->nch_pad + static_cast<size_t>(k) * CH + cl;
+                const int c = t->chan[static_cast<size_t>(k) * CH + cl];
+                int32_t base = 0;
+                int sw = D_J;  // padding channel: a zero row of X, read at offset 0
+                if (c < nchans) {
+                    int32_t lo = std::numeric_limits<int32_t>::max(), hi = 0;
+                    for (int d = d0; d < d1; ++d) {
+                        const int32_t s = table[static_cast<size_t>(d) * nchans + c];
+                        lo = std::min(lo, s);
+                        hi = std::max(hi, s);
+                    }
+                    base = lo - lo % A;
+                    sw = static_cast<int>(round_up(static_cast<int64_t>(D_J) + (hi - base), A));
+                } else {
+                    sw = static_cast<int>(round_up(D_J, A));
+                }
+                int32_t *q = t->blk.data() + slot * 4;
+                q[0] = c;
+                q[1] = base;
+                q[2] = sw * S;
+                q[3] = dst;
+                dst += sw * S;
             }
-            int32_t lo = std::numeric_limits<int32_t>::max(), hi = 0;
-            for (int d = d0; d < d1; ++d) {
-                const int32_t s = table[static_cast<size_t>(d) * nchans + c];
-                lo = std::min(lo, s);
-                hi = std::max(hi, s);
-            }
-            const int32_t base = lo & ~3;
-            const int words = static_cast<int>(round_up(static_cast<int64_t>(D_J) + (hi - base), 4));
-            t->blk_base[i] = base;
-            t->blk_len[i] = words * 4;
-            pitch_words = std::max(pitch_words, words);
-            per_jtile_bytes += t->blk_len[i];
+            rows_bytes = std::max(rows_bytes, dst);
+            per_jtile_bytes += dst;
         }
     }
-    t->pitch_words = pitch_words;
-    const int64_t ofs_stage_bytes = static_cast<int64_t>(D_DM) * CH * 4;
-    const int64_t stage_bytes = static_cast<int64_t>(CH) * pitch_words * 4 + ofs_stage_bytes;
+    t->rows_bytes = rows_bytes;
+    const int64_t ofs_stage_bytes = static_cast<int64_t>(D_DM) * CH * shape.OW;
+    const int64_t stage_bytes = rows_bytes + ofs_stage_bytes;
     const int64_t barrier_bytes = 1024;  // mbarriers + slack, see dd_kernels.cu
-    int nstage = static_cast<int>((smem_limit - barrier_bytes) / stage_bytes);
+    // NB CTAs per SM share the SM's shared memory (1 KB per CTA is reserved by the driver)
+    const int64_t cta_limit = shape.NB > 1 ? (smem_limit + 1024) / shape.NB - 1024 : smem_limit;
+    int nstage = static_cast<int>((cta_limit - barrier_bytes) / stage_bytes);
     nstage = std::min(nstage, std::min(8, std::max(t->nk, 2)));
     if (nstage < 2) return false;
     t->nstage = nstage;
@@ -114,24 +140,27 @@ bool build_tiling(const KernelShape &shape, int variant, const int32_t *table, i
     t->stage_bytes_total =
         (per_jtile_bytes + static_cast<int64_t>(t->ndb) * t->nk * ofs_stage_bytes) * t->ntj;
 
-    // ofs[b][k][dl][cl] = cl*pitch_bytes + 4*(s(d,c) - base(b,c)); DM rows past the end of the
+    // ofs[b][k][dl][cl] = dst(b,k,cl) + S*(s(d,c) - base(b,c)) (bytes, or /4 when OW == 2); DM rows past the end of the
     // plan repeat the block's last valid row (their results are computed and not stored).
-    t->ofs.assign(static_cast<size_t>(t->ndb) * t->nk * D_DM * CH, 0);
-    const int pitch_bytes = pitch_words * 4;
+    t->ofs.assign(static_cast<size_t>(t->ndb) * t->nk * D_DM * CH * shape.OW, 0);
     for (int b = 0; b < t->ndb; ++b)
         for (int k = 0; k < t->nk; ++k)
             for (int dl = 0; dl < D_DM; ++dl) {
                 const int d = std::min(ndm - 1, b * D_DM + dl);
-                int32_t *dst = t->ofs.data() +
-                               ((static_cast<size_t>(b) * t->nk + k) * D_DM + dl) * CH;
+                uint8_t *dst = t->ofs.data() +
+                               ((static_cast<size_t>(b) * t->nk + k) * D_DM + dl) * CH * shape.OW;
                 for (int cl = 0; cl < CH; ++cl) {
-                    const int c = k * CH + cl;
-                    int32_t o = cl * pitch_bytes;
-                    if (c < nchans) {
-                        const size_t i = static_cast<size_t>(b) * t->nch_pad + c;
-                        o += 4 * (table[static_cast<size_t>(d) * nchans + c] - t->blk_base[i]);
+                    const size_t slot = static_cast<size_t>(b) * t->nch_pad + static_cast<size_t>(k) * CH + cl;
+                    const int32_t *q = t->blk.data() + slot * 4;
+                    int32_t o = q[3];
+                    if (q[0] < nchans)
+                        o += S * (table[static_cast<size_t>(d) * nchans + q[0]] - q[1]);
+                    if (shape.OW == 2) {  // units of 4 bytes; < 2^16 because shared memory is < 256 KB
+                        const uint16_t v = static_cast<uint16_t>(o / 4);
+                        std::memcpy(dst + cl * 2, &v, 2);
+                    } else {
+                        std::memcpy(dst + cl * 4, &o, 4);
                     }
-                    dst[cl] = o;
                 }
             }
     return true;

@@ -10,18 +10,27 @@ namespace dd {
 
 // ---- host-side tiling of one plan --------------------------
 //
-// The time axis is re-indexed in 32-bit "words": word j of channel c carries LANES samples
-// of that channel, lane k being in[c][k*L + j].  Every lane of a word needs the SAME shift
-// for a given (DM, channel), so a shifted read is just a word-index offset -- no byte
-// alignment problem, whatever the shift.
+// The time axis is re-indexed in "superwords" of VW 32-bit words: superword j of channel c
+// carries LANES = VW * (4 | 2 | 1) samples of that channel, lane l being in[c][l*L + j]
+// (word v of the superword holds lanes v*LPW .. v*LPW + LPW-1, LPW = samples per 32-bit
+// word).  Every lane needs the SAME shift for a given (DM, channel), so a shifted read is a
+// superword-index offset: always aligned for LDS.32/64/128, whatever the shift (DESIGN.md
+// "Data layout").
 struct KernelShape {
     int mode;     // DD_U8 / DD_U16 / DD_F32
-    int lanes;    // 4 / 2 / 1
-    int RD, RW;   // DM trials and words per thread
+    int VW;       // 32-bit words per superword: 1, 2, 4 (LDS.32 / LDS.64 / LDS.128)
+    int RD, RJ;   // DM trials and superwords per thread
     int WD, WJ;   // consumer warps along DM and along j
-    int CH;       // channels per pipeline stage
+    int CH;       // channels per pipeline stage (multiple of 8, <= 32)
+    int FM;       // u8: which adds run as IMAD on the fma pipe (dd_kernels.cu)
+    int NB;       // CTAs per SM the shared-memory ring is sized for
+    int OW;       // bytes per shared-memory offset entry: 4 (byte offsets) or 2 (units of 4 bytes)
+    int tune;     // 0: eligible for automatic selection; 1: DD_FORCE_VARIANT only
+    int lpw() const { return mode == DD_U8 ? 4 : (mode == DD_U16 ? 2 : 1); }
+    int lanes() const { return VW * lpw(); }
+    int sw_bytes() const { return VW * 4; }
     int D_DM() const { return RD * WD; }
-    int D_J() const { return RW * WJ * 32; }
+    int D_J() const { return RJ * WJ * 32; }
     int threads() const { return (WD * WJ + 1) * 32; }  // + 1 producer warp
 };
 
@@ -29,16 +38,21 @@ struct Tiling {
     KernelShape shape{};
     int variant = -1;          // index into the compiled kernel table
     int64_t L = 0;             // lane stride (samples), multiple of 16
-    int64_t Lw = 0;            // words per row of the interleaved workspace X
+    int64_t Lw = 0;            // superwords per row of the interleaved workspace X
     int nch_pad = 0;           // nchans rounded up to CH (padding rows of X stay zero)
     int ndb = 0, ntj = 0, nk = 0;  // DM blocks, j tiles, channel stages
-    int pitch_words = 0;       // shared-memory row pitch (words)
+    int rows_bytes = 0;        // bytes of channel windows in one stage buffer (multiple of 16)
     int nstage = 0;
     int64_t smem_bytes = 0;
     int64_t stage_bytes_total = 0;  // global->shared bytes per launch (DD_INFO_STAGE_BYTES)
-    std::vector<int32_t> ofs;       // [ndb][nk][D_DM][CH]  byte offset inside a stage buffer
-    std::vector<int32_t> blk_base;  // [ndb][nch_pad]       first staged word (multiple of 4)
-    std::vector<int32_t> blk_len;   // [ndb][nch_pad]       staged bytes (multiple of 16)
+    // Stage k of DM block b holds the CH channels chan[k*CH .. k*CH+CH): a fixed permutation
+    // that pairs short windows (high frequencies) with long ones (low frequencies) so that
+    // every stage needs about the same number of bytes.
+    std::vector<int32_t> chan;      // [nch_pad]            channel staged in slot k*CH + cl
+    std::vector<uint8_t> ofs;       // [ndb][nk][D_DM][CH] entries of OW bytes: offset inside a stage buffer
+    // [ndb][nch_pad] per slot: x = channel, y = first staged superword (16-B aligned address),
+    // z = staged bytes (multiple of 16), w = byte offset of the window inside the stage buffer
+    std::vector<int32_t> blk;       // 4 ints per slot
 };
 
 // Eq. 1 / Eq. 7 on the host; returns a dd_status.
@@ -53,17 +67,17 @@ bool build_tiling(const KernelShape &shape, int variant, const int32_t *table, i
 // ---- device side -------------------------------------------------------------------------
 struct KernelParams {
     const uint32_t *X;
-    const int32_t *ofs;
-    const int32_t *blk_base;
-    const int32_t *blk_len;
+    const void *ofs;      // [ndb][nk][D_DM][CH] entries of OW bytes
+    const int32_t *blk;   // 4 ints per slot (read as int4)
     void *out;
     int64_t out_len;
-    int64_t Lw;
+    int64_t Lw;        // superwords per row of X
     int64_t L;
     int ndm, nch_pad, nk, ndb, ntj;
-    int pitch_bytes;   // smem row pitch
+    int rows_bytes;    // channel windows of one stage; the stage's offset table follows
     int nstage;
-    int stage_bytes;   // CH*pitch_bytes + D_DM*CH*4, multiple of 16
+    int stage_bytes;   // rows_bytes + D_DM*CH*OW, multiple of 16
+    uint32_t one;      // 1, opaque to ptxas
 };
 
 struct InterleaveParams {
@@ -71,7 +85,7 @@ struct InterleaveParams {
     uint32_t *X;
     int64_t nsamps, L, Lw;
     int nchans;
-    int nchunk;  // blocks per channel row: ceil(Lw / (4 * 256))
+    int nchunk;  // blocks per channel row: ceil(Lw / (4 * 256)), a thread makes 4 superwords
 };
 
 int num_variants();
@@ -80,6 +94,6 @@ const KernelShape &variant_shape(int v);
 int variant_prepare(int v, int smem_bytes);
 // Launch the main kernel / the interleave pre-pass on `stream`; return cudaError_t as int.
 int launch_dedisperse(int v, const KernelParams &p, int grid, int smem_bytes, void *stream);
-int launch_interleave(int mode, const InterleaveParams &p, void *stream);
+int launch_interleave(int mode, int VW, const InterleaveParams &p, void *stream);
 
 }  // namespace dd

@@ -70,17 +70,33 @@ __device__ __forceinline__ uint32_t odd_bytes(uint32_t w)
 }
 
 // ------------------------------------------------------------------ per-mode accumulators
-template <int MODE>
+template <int MODE, int FM>
 struct Acc;
 
-template <>
-struct Acc<DD_U8> {
+// FM (u8 only) = which adds are issued as IMAD (x * one + acc, `one` a runtime 1 that ptxas
+// cannot fold) on the fma pipe instead of IADD3 on the alu pipe:
+//   0 none; 1 W += x (both words); 2 O += odd(x) (both words); 3 W += x for the second word only
+template <int FM>
+struct Acc<DD_U8, FM> {
     uint32_t W = 0, O = 0;           // packed, flushed every <= 256 channels
     uint32_t a0 = 0, a1 = 0, a2 = 0, a3 = 0;
-    __device__ __forceinline__ void add2(uint32_t x, uint32_t y)
+    __device__ __forceinline__ void add2(uint32_t x, uint32_t y, uint32_t one)
     {
-        W = W + x + y;
-        O = O + odd_bytes(x) + odd_bytes(y);
+        if (FM == 1) {
+            W = x * one + W;
+            W = y * one + W;
+        } else if (FM == 3) {
+            W = W + x;
+            W = y * one + W;
+        } else {
+            W = W + x + y;
+        }
+        if (FM == 2) {
+            O = odd_bytes(x) * one + O;
+            O = odd_bytes(y) * one + O;
+        } else {
+            O = O + odd_bytes(x) + odd_bytes(y);
+        }
     }
     __device__ __forceinline__ void flush()
     {
@@ -95,10 +111,10 @@ struct Acc<DD_U8> {
     static constexpr bool kNeedsFlush = true;
 };
 
-template <>
-struct Acc<DD_U16> {
+template <int FM>
+struct Acc<DD_U16, FM> {
     uint32_t W = 0, H = 0;
-    __device__ __forceinline__ void add2(uint32_t x, uint32_t y)
+    __device__ __forceinline__ void add2(uint32_t x, uint32_t y, uint32_t)
     {
         W = W + x + y;
         H = H + (x >> 16) + (y >> 16);
@@ -107,10 +123,10 @@ struct Acc<DD_U16> {
     static constexpr bool kNeedsFlush = false;
 };
 
-template <>
-struct Acc<DD_F32> {
+template <int FM>
+struct Acc<DD_F32, FM> {
     float s = 0.f;
-    __device__ __forceinline__ void add2(uint32_t x, uint32_t y)
+    __device__ __forceinline__ void add2(uint32_t x, uint32_t y, uint32_t)
     {
         s += __uint_as_float(x);
         s += __uint_as_float(y);
@@ -120,19 +136,73 @@ struct Acc<DD_F32> {
 };
 
 // ------------------------------------------------------------------ main kernel
-template <int MODE, int RD, int RW, int WD, int WJ, int CH>
-__global__ void __launch_bounds__((WD * WJ + 1) * 32, 1) dedisperse_kernel(const KernelParams p)
+// One shared-memory load of VW words (LDS.32 / LDS.64 / LDS.128) at a 32-bit shared-space
+// address plus a compile-time byte offset.
+template <int VW>
+struct SW;
+template <>
+struct SW<1> {
+    uint32_t w[1];
+    template <int IMM>
+    __device__ __forceinline__ void load(uint32_t a)
+    {
+        asm volatile("ld.shared.u32 %0, [%1+%2];" : "=r"(w[0]) : "r"(a), "n"(IMM) : "memory");
+    }
+};
+template <>
+struct SW<2> {
+    uint32_t w[2];
+    template <int IMM>
+    __device__ __forceinline__ void load(uint32_t a)
+    {
+        asm volatile("ld.shared.v2.u32 {%0,%1}, [%2+%3];" : "=r"(w[0]), "=r"(w[1]) : "r"(a), "n"(IMM) : "memory");
+    }
+};
+template <>
+struct SW<4> {
+    uint32_t w[4];
+    template <int IMM>
+    __device__ __forceinline__ void load(uint32_t a)
+    {
+        asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4+%5];"
+                     : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3])
+                     : "r"(a), "n"(IMM)
+                     : "memory");
+    }
+};
+
+// RJ superword loads of one channel row (stride 32 superwords) added into acc[.][.].
+template <int MODE, int VW, int RJ, int FM, int I = 0>
+struct RowPair {
+    static __device__ __forceinline__ void run(Acc<MODE, FM> (&acc)[RJ][VW], uint32_t a0, uint32_t a1,
+                                               uint32_t one)
+    {
+        SW<VW> x, y;
+        x.template load<I * 32 * VW * 4>(a0);
+        y.template load<I * 32 * VW * 4>(a1);
+#pragma unroll
+        for (int v = 0; v < VW; ++v) acc[I][v].add2(x.w[v], y.w[v], one);
+        RowPair<MODE, VW, RJ, FM, I + 1>::run(acc, a0, a1, one);
+    }
+};
+template <int MODE, int VW, int RJ, int FM>
+struct RowPair<MODE, VW, RJ, FM, RJ> {
+    static __device__ __forceinline__ void run(Acc<MODE, FM> (&)[RJ][VW], uint32_t, uint32_t, uint32_t) {}
+};
+
+template <int MODE, int VW, int RD, int RJ, int WD, int WJ, int CH, int FM, int NB, int OW>
+__global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(const KernelParams p)
 {
     constexpr int NCW = WD * WJ;  // consumer warps
     constexpr int D_DM = RD * WD;
-    constexpr int D_J = RW * WJ * 32;
-    constexpr int LANES = MODE == DD_U8 ? 4 : (MODE == DD_U16 ? 2 : 1);
-    static_assert(CH % 4 == 0 && CH <= 32, "CH: multiple of 4, one producer lane per channel");
-    static_assert(256 % CH == 0, "u8 flush period must be a whole number of stages");
+    constexpr int D_J = RJ * WJ * 32;  // superwords
+    constexpr int S = VW * 4;          // bytes per superword
+    constexpr int LPW = MODE == DD_U8 ? 4 : (MODE == DD_U16 ? 2 : 1);
+    static_assert(CH % (16 / OW) == 0 && CH <= 32, "CH: whole LDS.128 offset loads, one producer lane per channel");
 
     extern __shared__ __align__(128) unsigned char smem[];
-    // [0, 1024): mbarriers full[nstage], empty[nstage]; then nstage stage buffers, each
-    // CH rows of pitch_bytes followed by the D_DM x CH int32 offset table.
+    // [0, 1024): mbarriers full[nstage], empty[nstage]; then nstage stage buffers, each the
+    // packed channel windows (rows_bytes) followed by the D_DM x CH offset table (OW = 4: byte offsets; OW = 2: uint16 in units of 4 bytes).
     const uint32_t bar_full = smem_u32(smem);
     const uint32_t bar_empty = bar_full + 8u * 8u;
     unsigned char *stage0 = smem + 1024;
@@ -153,31 +223,32 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, 1) dedisperse_kernel(const
     __syncthreads();
 
     if (warp == NCW) {
-        // ===================== producer warp: lane l stages channel l of each stage
-        const int32_t *base_row = p.blk_base + static_cast<size_t>(b) * p.nch_pad;
-        const int32_t *len_row = p.blk_len + static_cast<size_t>(b) * p.nch_pad;
-        const int32_t *ofs_blk = p.ofs + static_cast<size_t>(b) * p.nk * (D_DM * CH);
+        // ===================== producer warp: lane l stages slot l of each stage
+        const int4 *blk = reinterpret_cast<const int4 *>(p.blk) + static_cast<size_t>(b) * p.nch_pad;
+        const unsigned char *ofs_blk =
+            static_cast<const unsigned char *>(p.ofs) + static_cast<size_t>(b) * p.nk * (D_DM * CH * OW);
+        const unsigned char *Xb = reinterpret_cast<const unsigned char *>(p.X);
         int s = 0;
         uint32_t phase = 0;
+        int4 q = make_int4(0, 0, 0, 0);
+        if (lane < CH) q = blk[lane];
         for (int k = 0; k < p.nk; ++k) {
-            uint32_t bytes = 0;
-            const uint32_t *src = nullptr;
-            if (lane < CH) {
-                const int c = k * CH + lane;
-                bytes = static_cast<uint32_t>(len_row[c]);
-                src = p.X + static_cast<size_t>(c) * p.Lw + j0 + base_row[c];
-            }
-            const uint32_t total = __reduce_add_sync(0xffffffffu, bytes) + D_DM * CH * 4;
+            const uint32_t bytes = static_cast<uint32_t>(q.z);
+            const unsigned char *src =
+                Xb + (static_cast<size_t>(q.x) * p.Lw + j0 + q.y) * S;
+            const uint32_t dsto = static_cast<uint32_t>(q.w);
+            if (k + 1 < p.nk && lane < CH) q = blk[(k + 1) * CH + lane];  // prefetch next stage's slots
+            const uint32_t total = __reduce_add_sync(0xffffffffu, bytes) + D_DM * CH * OW;
             if (k >= nstage) mbar_wait(bar_empty + 8u * s, phase ^ 1u);
             const uint32_t full = bar_full + 8u * s;
             const uint32_t dst = smem_u32(stage0) + static_cast<uint32_t>(s) * p.stage_bytes;
             if (lane == 0) {
                 mbar_arrive_expect_tx(full, total);
-                bulk_g2s(dst + CH * p.pitch_bytes, ofs_blk + static_cast<size_t>(k) * (D_DM * CH),
-                         D_DM * CH * 4, full);
+                bulk_g2s(dst + p.rows_bytes, ofs_blk + static_cast<size_t>(k) * (D_DM * CH * OW),
+                         D_DM * CH * OW, full);
             }
             __syncwarp();
-            if (lane < CH) bulk_g2s(dst + lane * p.pitch_bytes, src, bytes, full);
+            if (lane < CH) bulk_g2s(dst + dsto, src, bytes, full);
             if (++s == nstage) {
                 s = 0;
                 phase ^= 1u;
@@ -188,41 +259,63 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, 1) dedisperse_kernel(const
 
     // ========================= consumer warps
     const int wd = warp / WJ, wj = warp % WJ;
-    Acc<MODE> acc[RD][RW];
-    const uint32_t lane_byte = static_cast<uint32_t>((wj * RW * 32 + lane) * 4);
+    Acc<MODE, FM> acc[RD][RJ][VW];
+    const uint32_t one = p.one;
+    const uint32_t four = one * 4u;
+    const uint32_t lane_byte = static_cast<uint32_t>((wj * RJ * 32 + lane) * S);
+    const uint32_t stage_u32 = smem_u32(stage0);
 
     int s = 0;
+    int since_flush = 0;
     uint32_t phase = 0;
     for (int k = 0; k < p.nk; ++k) {
         mbar_wait(bar_full + 8u * s, phase);
-        const unsigned char *stage = stage0 + static_cast<size_t>(s) * p.stage_bytes;
-        const unsigned char *rows = stage + lane_byte;
-        const int4 *otab = reinterpret_cast<const int4 *>(stage + CH * p.pitch_bytes) +
-                           (wd * RD) * (CH / 4);
+        const uint32_t stage = stage_u32 + static_cast<uint32_t>(s) * p.stage_bytes;
+        const uint32_t rows = stage + lane_byte;
+        const uint32_t otab = stage + p.rows_bytes + (wd * RD) * (CH * OW);
+        // One LDS.128 fetches 16 / OW offsets per DM trial (a broadcast: the row is warp-uniform).
+        // address = offset * scale + rows as IMAD on the fma pipe (`one` is opaque to ptxas).
+        constexpr int NPER = 16 / OW;
 #pragma unroll
-        for (int c4 = 0; c4 < CH / 4; ++c4) {
-            int4 o[RD];
+        for (int cg = 0; cg < CH / NPER; ++cg) {
+            uint32_t o[RD][4];
 #pragma unroll
-            for (int r = 0; r < RD; ++r) o[r] = otab[r * (CH / 4) + c4];
+            for (int r = 0; r < RD; ++r)
+                asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];"
+                             : "=r"(o[r][0]), "=r"(o[r][1]), "=r"(o[r][2]), "=r"(o[r][3])
+                             : "r"(otab + r * (CH * OW) + cg * 16)
+                             : "memory");
 #pragma unroll
             for (int r = 0; r < RD; ++r) {
-                const uint32_t *q0 = reinterpret_cast<const uint32_t *>(rows + o[r].x);
-                const uint32_t *q1 = reinterpret_cast<const uint32_t *>(rows + o[r].y);
-                const uint32_t *q2 = reinterpret_cast<const uint32_t *>(rows + o[r].z);
-                const uint32_t *q3 = reinterpret_cast<const uint32_t *>(rows + o[r].w);
+                if constexpr (OW == 2) {
 #pragma unroll
-                for (int i = 0; i < RW; ++i) acc[r][i].add2(q0[i * 32], q1[i * 32]);
+                    for (int h = 0; h < 4; ++h) {
+                        const uint32_t a0 = (o[r][h] & 0xffffu) * four + rows;
+                        const uint32_t a1 = (o[r][h] >> 16) * four + rows;
+                        RowPair<MODE, VW, RJ, FM>::run(acc[r], a0, a1, one);
+                    }
+                } else {
 #pragma unroll
-                for (int i = 0; i < RW; ++i) acc[r][i].add2(q2[i * 32], q3[i * 32]);
+                    for (int h = 0; h < 2; ++h) {
+                        const uint32_t a0 = o[r][2 * h] * one + rows;
+                        const uint32_t a1 = o[r][2 * h + 1] * one + rows;
+                        RowPair<MODE, VW, RJ, FM>::run(acc[r], a0, a1, one);
+                    }
+                }
             }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_empty + 8u * s);
-        if (Acc<MODE>::kNeedsFlush && (((k + 1) * CH) & 255) == 0) {
+        // u8: the packed 16-bit lanes hold at most 256 channels (256 * 255 < 2^16) between flushes
+        since_flush += CH;
+        if (Acc<MODE, FM>::kNeedsFlush && since_flush + CH > 256) {
+            since_flush = 0;
 #pragma unroll
             for (int r = 0; r < RD; ++r)
 #pragma unroll
-                for (int i = 0; i < RW; ++i) acc[r][i].flush();
+                for (int i = 0; i < RJ; ++i)
+#pragma unroll
+                    for (int v = 0; v < VW; ++v) acc[r][i][v].flush();
         }
         if (++s == nstage) {
             s = 0;
@@ -230,114 +323,132 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, 1) dedisperse_kernel(const
         }
     }
 
-    // ========================= store (a7): lane k of word j is output sample k*L + j
+    // ========================= store (a7): lane l of superword j is output sample l*L + j
 #pragma unroll
     for (int r = 0; r < RD; ++r) {
         const int d = b * D_DM + wd * RD + r;
         if (d >= p.ndm) continue;
 #pragma unroll
-        for (int i = 0; i < RW; ++i) {
-            const int64_t j = j0 + (wj * RW + i) * 32 + lane;
+        for (int i = 0; i < RJ; ++i) {
+            const int64_t j = j0 + (wj * RJ + i) * 32 + lane;
             if (j >= p.L) continue;
-            if constexpr (MODE == DD_U8) {
-                Acc<DD_U8> &a = acc[r][i];
-                a.flush();
-                uint32_t *o = static_cast<uint32_t *>(p.out) + static_cast<size_t>(d) * p.out_len;
-                const uint32_t v[4] = {a.a0, a.a1, a.a2, a.a3};
 #pragma unroll
-                for (int l = 0; l < LANES; ++l) {
-                    const int64_t t = l * p.L + j;
-                    if (t < p.out_len) o[t] = v[l];
+            for (int v = 0; v < VW; ++v) {
+                uint32_t val[LPW];
+                if constexpr (MODE == DD_U8) {
+                    Acc<DD_U8, FM> &a = acc[r][i][v];
+                    a.flush();
+                    val[0] = a.a0;
+                    val[1] = a.a1;
+                    val[2] = a.a2;
+                    val[3] = a.a3;
+                } else if constexpr (MODE == DD_U16) {
+                    Acc<DD_U16, FM> &a = acc[r][i][v];
+                    val[0] = a.W - (a.H << 16);
+                    val[1] = a.H;
+                } else {
+                    val[0] = __float_as_uint(acc[r][i][v].s);
                 }
-            } else if constexpr (MODE == DD_U16) {
-                Acc<DD_U16> &a = acc[r][i];
                 uint32_t *o = static_cast<uint32_t *>(p.out) + static_cast<size_t>(d) * p.out_len;
-                const uint32_t v[2] = {a.W - (a.H << 16), a.H};
 #pragma unroll
-                for (int l = 0; l < LANES; ++l) {
-                    const int64_t t = l * p.L + j;
-                    if (t < p.out_len) o[t] = v[l];
+                for (int l = 0; l < LPW; ++l) {
+                    const int64_t t = static_cast<int64_t>(v * LPW + l) * p.L + j;
+                    if (t < p.out_len) o[t] = val[l];
                 }
-            } else {
-                Acc<DD_F32> &a = acc[r][i];
-                float *o = static_cast<float *>(p.out) + static_cast<size_t>(d) * p.out_len;
-                if (j < p.out_len) o[j] = a.s;
             }
         }
     }
 }
 
 // ------------------------------------------------------------------ interleave pre-pass
-// One thread makes four consecutive words (one 16-byte store).  Reads past the end of a
-// row (t >= nsamps) give 0; such lanes only feed outputs that are never stored.
+// One thread makes four consecutive superwords (16*VW bytes, VW 16-byte stores) of one
+// channel from LANES four-sample segments of the input row.  Reads past the end of a row
+// (t >= nsamps) give 0; such lanes only feed outputs that are never stored.
 template <typename T>
 __device__ __forceinline__ uint32_t sample_or_zero(const T *row, int64_t t, int64_t nsamps)
 {
     return t < nsamps ? static_cast<uint32_t>(row[t]) : 0u;
 }
 
-template <int MODE>
+template <int MODE, int VW>
 __global__ void __launch_bounds__(256) interleave_kernel(const InterleaveParams p)
 {
     const int c = static_cast<int>(blockIdx.x / p.nchunk);
     const int64_t j = (static_cast<int64_t>(blockIdx.x % p.nchunk) * blockDim.x + threadIdx.x) * 4;
     if (j >= p.Lw) return;
-    uint4 w;
+    uint32_t w[4 * VW];  // w[q * VW + v] = word v of superword j + q
     if (MODE == DD_U8) {
         const uint8_t *row = static_cast<const uint8_t *>(p.in) + static_cast<size_t>(c) * p.nsamps;
         const bool aligned = (reinterpret_cast<uintptr_t>(row) & 3u) == 0;
-        uint32_t seg[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const int64_t t = k * p.L + j;
-            if (aligned && t + 3 < p.nsamps) {
-                seg[k] = *reinterpret_cast<const uint32_t *>(row + t);
-            } else {
-                seg[k] = sample_or_zero(row, t, p.nsamps) | sample_or_zero(row, t + 1, p.nsamps) << 8 |
-                         sample_or_zero(row, t + 2, p.nsamps) << 16 |
-                         sample_or_zero(row, t + 3, p.nsamps) << 24;
+        for (int v = 0; v < VW; ++v) {
+            uint32_t seg[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int64_t t = (v * 4 + k) * p.L + j;
+                if (aligned && t + 3 < p.nsamps) {
+                    seg[k] = *reinterpret_cast<const uint32_t *>(row + t);
+                } else {
+                    seg[k] = sample_or_zero(row, t, p.nsamps) | sample_or_zero(row, t + 1, p.nsamps) << 8 |
+                             sample_or_zero(row, t + 2, p.nsamps) << 16 |
+                             sample_or_zero(row, t + 3, p.nsamps) << 24;
+                }
             }
+            // 4x4 byte transpose: word q gets byte q of each segment
+            const uint32_t t01l = __byte_perm(seg[0], seg[1], 0x5140);  // a0 b0 a1 b1
+            const uint32_t t01h = __byte_perm(seg[0], seg[1], 0x7362);  // a2 b2 a3 b3
+            const uint32_t t23l = __byte_perm(seg[2], seg[3], 0x5140);
+            const uint32_t t23h = __byte_perm(seg[2], seg[3], 0x7362);
+            w[0 * VW + v] = __byte_perm(t01l, t23l, 0x5410);
+            w[1 * VW + v] = __byte_perm(t01l, t23l, 0x7632);
+            w[2 * VW + v] = __byte_perm(t01h, t23h, 0x5410);
+            w[3 * VW + v] = __byte_perm(t01h, t23h, 0x7632);
         }
-        // 4x4 byte transpose: word n gets byte n of each segment
-        const uint32_t t01l = __byte_perm(seg[0], seg[1], 0x5140);  // a0 b0 a1 b1
-        const uint32_t t01h = __byte_perm(seg[0], seg[1], 0x7362);  // a2 b2 a3 b3
-        const uint32_t t23l = __byte_perm(seg[2], seg[3], 0x5140);
-        const uint32_t t23h = __byte_perm(seg[2], seg[3], 0x7362);
-        w.x = __byte_perm(t01l, t23l, 0x5410);
-        w.y = __byte_perm(t01l, t23l, 0x7632);
-        w.z = __byte_perm(t01h, t23h, 0x5410);
-        w.w = __byte_perm(t01h, t23h, 0x7632);
     } else if (MODE == DD_U16) {
         const uint16_t *row = static_cast<const uint16_t *>(p.in) + static_cast<size_t>(c) * p.nsamps;
         const bool aligned = (reinterpret_cast<uintptr_t>(row) & 7u) == 0;
-        uint2 seg[2];
 #pragma unroll
-        for (int k = 0; k < 2; ++k) {
-            const int64_t t = k * p.L + j;
-            if (aligned && t + 3 < p.nsamps) {
-                seg[k] = *reinterpret_cast<const uint2 *>(row + t);
-            } else {
-                seg[k].x = sample_or_zero(row, t, p.nsamps) | sample_or_zero(row, t + 1, p.nsamps) << 16;
-                seg[k].y = sample_or_zero(row, t + 2, p.nsamps) | sample_or_zero(row, t + 3, p.nsamps) << 16;
+        for (int v = 0; v < VW; ++v) {
+            uint2 seg[2];
+#pragma unroll
+            for (int k = 0; k < 2; ++k) {
+                const int64_t t = (v * 2 + k) * p.L + j;
+                if (aligned && t + 3 < p.nsamps) {
+                    seg[k] = *reinterpret_cast<const uint2 *>(row + t);
+                } else {
+                    seg[k].x = sample_or_zero(row, t, p.nsamps) | sample_or_zero(row, t + 1, p.nsamps) << 16;
+                    seg[k].y = sample_or_zero(row, t + 2, p.nsamps) | sample_or_zero(row, t + 3, p.nsamps) << 16;
+                }
             }
+            w[0 * VW + v] = __byte_perm(seg[0].x, seg[1].x, 0x5410);
+            w[1 * VW + v] = __byte_perm(seg[0].x, seg[1].x, 0x7632);
+            w[2 * VW + v] = __byte_perm(seg[0].y, seg[1].y, 0x5410);
+            w[3 * VW + v] = __byte_perm(seg[0].y, seg[1].y, 0x7632);
         }
-        w.x = __byte_perm(seg[0].x, seg[1].x, 0x5410);
-        w.y = __byte_perm(seg[0].x, seg[1].x, 0x7632);
-        w.z = __byte_perm(seg[0].y, seg[1].y, 0x5410);
-        w.w = __byte_perm(seg[0].y, seg[1].y, 0x7632);
     } else {
         const uint32_t *row = static_cast<const uint32_t *>(p.in) + static_cast<size_t>(c) * p.nsamps;
         const bool aligned = (reinterpret_cast<uintptr_t>(row) & 15u) == 0;
-        if (aligned && j + 3 < p.nsamps) {
-            w = *reinterpret_cast<const uint4 *>(row + j);
-        } else {
-            w.x = sample_or_zero(row, j, p.nsamps);
-            w.y = sample_or_zero(row, j + 1, p.nsamps);
-            w.z = sample_or_zero(row, j + 2, p.nsamps);
-            w.w = sample_or_zero(row, j + 3, p.nsamps);
+#pragma unroll
+        for (int v = 0; v < VW; ++v) {
+            const int64_t t = v * p.L + j;
+            uint4 seg;
+            if (aligned && t + 3 < p.nsamps) {
+                seg = *reinterpret_cast<const uint4 *>(row + t);
+            } else {
+                seg.x = sample_or_zero(row, t, p.nsamps);
+                seg.y = sample_or_zero(row, t + 1, p.nsamps);
+                seg.z = sample_or_zero(row, t + 2, p.nsamps);
+                seg.w = sample_or_zero(row, t + 3, p.nsamps);
+            }
+            w[0 * VW + v] = seg.x;
+            w[1 * VW + v] = seg.y;
+            w[2 * VW + v] = seg.z;
+            w[3 * VW + v] = seg.w;
         }
     }
-    *reinterpret_cast<uint4 *>(p.X + static_cast<size_t>(c) * p.Lw + j) = w;
+    uint4 *dst = reinterpret_cast<uint4 *>(p.X + (static_cast<size_t>(c) * p.Lw + j) * VW);
+#pragma unroll
+    for (int i = 0; i < VW; ++i) dst[i] = make_uint4(w[4 * i], w[4 * i + 1], w[4 * i + 2], w[4 * i + 3]);
 }
 
 // ------------------------------------------------------------------ variant table
@@ -347,26 +458,39 @@ struct Variant {
     KernelFn fn;
 };
 
-#define DD_VARIANT(MODE, LANES, RD, RW, WD, WJ, CH)               \
-    {                                                             \
-        {MODE, LANES, RD, RW, WD, WJ, CH}, dedisperse_kernel<MODE, RD, RW, WD, WJ, CH> \
+#define DD_VARIANT(MODE, VW, RD, RJ, WD, WJ, CH, FM, NB, OW, TUNE)         \
+    {                                                                      \
+        {MODE, VW, RD, RJ, WD, WJ, CH, FM, NB, OW, TUNE},                  \
+            dedisperse_kernel<MODE, VW, RD, RJ, WD, WJ, CH, FM, NB, OW>    \
     }
 
 // Ordered per mode from the largest DM block to the smallest; dd_plan_create takes the
-// first whose shared-memory ring fits (smaller DM blocks = shorter staged windows).
+// first with TUNE == 0 whose shared-memory ring fits (smaller DM blocks = shorter staged
+// windows; smaller CH = smaller stages).  TUNE == 1 entries are reachable through the
+// DD_FORCE_VARIANT environment variable only (A/B measurements, profiles/).
+// u8: LDS.64 superwords, 12 DM warps x 6 superwords, odd-lane adds on the fma pipe (FM = 2):
+// the r01 sweep (profiles/r01_tuning.md) measured 58.0 ms on the headline config against
+// 68.3 ms for the LDS.32 / 16-warp / all-alu shape (entry 5).
 const Variant kVariants[] = {
-    DD_VARIANT(DD_U8, 4, 1, 8, 16, 1, 16),
-    DD_VARIANT(DD_U8, 4, 1, 8, 8, 2, 16),
-    DD_VARIANT(DD_U8, 4, 1, 8, 4, 4, 16),
-    DD_VARIANT(DD_U8, 4, 1, 8, 1, 16, 16),
-    DD_VARIANT(DD_U16, 2, 2, 8, 16, 1, 16),
-    DD_VARIANT(DD_U16, 2, 1, 8, 16, 1, 16),
-    DD_VARIANT(DD_U16, 2, 1, 8, 4, 4, 16),
-    DD_VARIANT(DD_U16, 2, 1, 8, 1, 16, 16),
-    DD_VARIANT(DD_F32, 1, 2, 8, 16, 1, 16),
-    DD_VARIANT(DD_F32, 1, 1, 8, 16, 1, 16),
-    DD_VARIANT(DD_F32, 1, 1, 8, 4, 4, 16),
-    DD_VARIANT(DD_F32, 1, 1, 8, 1, 16, 16),
+    //         mode  VW RD RJ  WD  WJ  CH FM NB OW tune
+    DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 2, 1, 4, 0),   // 0
+    DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 16, 2, 1, 4, 0),   // 1
+    DD_VARIANT(DD_U8, 2, 1, 6, 6, 2, 16, 2, 1, 4, 0),    // 2
+    DD_VARIANT(DD_U8, 2, 1, 6, 3, 4, 16, 2, 1, 4, 0),    // 3
+    DD_VARIANT(DD_U8, 2, 1, 6, 1, 12, 8, 2, 1, 4, 0),    // 4
+    DD_VARIANT(DD_U8, 1, 1, 8, 16, 1, 16, 0, 1, 4, 1),   // 5  r01 first shape (A/B only)
+    DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 1, 1, 4, 1),   // 6  W on fma instead of O (A/B only)
+    DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 0, 1, 4, 1),   // 7  all adds on alu (A/B only)
+    DD_VARIANT(DD_U16, 1, 2, 8, 16, 1, 16, 0, 1, 4, 0),  // 8
+    DD_VARIANT(DD_U16, 1, 1, 8, 16, 1, 16, 0, 1, 4, 0),  // 9
+    DD_VARIANT(DD_U16, 1, 1, 8, 4, 4, 16, 0, 1, 4, 0),   // 10
+    DD_VARIANT(DD_U16, 1, 1, 8, 1, 16, 8, 0, 1, 4, 0),   // 11
+    DD_VARIANT(DD_U16, 2, 2, 4, 16, 1, 16, 0, 1, 4, 1),  // 12 LDS.64 (A/B only)
+    DD_VARIANT(DD_F32, 1, 2, 8, 16, 1, 16, 0, 1, 2, 0),  // 13
+    DD_VARIANT(DD_F32, 1, 1, 8, 16, 1, 16, 0, 1, 2, 0),  // 14
+    DD_VARIANT(DD_F32, 1, 1, 8, 4, 4, 16, 0, 1, 2, 0),   // 15
+    DD_VARIANT(DD_F32, 1, 1, 8, 1, 16, 8, 0, 1, 2, 0),   // 16
+    DD_VARIANT(DD_F32, 1, 2, 8, 16, 1, 16, 0, 1, 4, 1),  // 17 32-bit offsets (A/B only)
 };
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 
@@ -389,16 +513,27 @@ int launch_dedisperse(int v, const KernelParams &p, int grid, int smem_bytes, vo
     return static_cast<int>(cudaGetLastError());
 }
 
-int launch_interleave(int mode, const InterleaveParams &p, void *stream)
+template <int VW>
+static void launch_interleave_vw(int mode, const InterleaveParams &p, unsigned grid, cudaStream_t st)
+{
+    if (mode == DD_U8)
+        interleave_kernel<DD_U8, VW><<<grid, 256, 0, st>>>(p);
+    else if (mode == DD_U16)
+        interleave_kernel<DD_U16, VW><<<grid, 256, 0, st>>>(p);
+    else
+        interleave_kernel<DD_F32, VW><<<grid, 256, 0, st>>>(p);
+}
+
+int launch_interleave(int mode, int VW, const InterleaveParams &p, void *stream)
 {
     const unsigned grid = static_cast<unsigned>(static_cast<int64_t>(p.nchunk) * p.nchans);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if (mode == DD_U8)
-        interleave_kernel<DD_U8><<<grid, 256, 0, st>>>(p);
-    else if (mode == DD_U16)
-        interleave_kernel<DD_U16><<<grid, 256, 0, st>>>(p);
+    if (VW == 1)
+        launch_interleave_vw<1>(mode, p, grid, st);
+    else if (VW == 2)
+        launch_interleave_vw<2>(mode, p, grid, st);
     else
-        interleave_kernel<DD_F32><<<grid, 256, 0, st>>>(p);
+        launch_interleave_vw<4>(mode, p, grid, st);
     return static_cast<int>(cudaGetLastError());
 }
 
