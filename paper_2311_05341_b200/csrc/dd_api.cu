@@ -24,6 +24,10 @@ struct dd_plan {
     int64_t workspace_bytes = 0;
     // dd_execute_host buffers (lazy)
     void *d_in_own = nullptr, *d_out_own = nullptr;
+    static constexpr int kHostChunks = 8;
+    bool host_made = false;
+    cudaStream_t st_h2d = nullptr, st_d2h = nullptr;
+    cudaEvent_t ev_in[kHostChunks + 1] = {}, ev_done[kHostChunks + 1] = {};
     // optional per-kernel timing (dd_plan_set_timing): ring of event triples
     static constexpr int kRing = 64;
     bool timing = false;
@@ -51,6 +55,12 @@ void free_device(dd_plan *p)
         if (p->ev_made)
             for (auto &triple : p->ev)
                 for (cudaEvent_t e : triple) cudaEventDestroy(e);
+        if (p->host_made) {
+            for (cudaEvent_t e : p->ev_in) cudaEventDestroy(e);
+            for (cudaEvent_t e : p->ev_done) cudaEventDestroy(e);
+            cudaStreamDestroy(p->st_h2d);
+            cudaStreamDestroy(p->st_d2h);
+        }
         if (cur >= 0 && cur != p->device) cudaSetDevice(cur);
     }
 }
@@ -184,49 +194,80 @@ int dd_plan_shift_table(const dd_plan *plan, const int32_t **table, int64_t *out
     return DD_OK;
 }
 
+}  // extern "C"
+
+namespace {
+
+// X columns (superwords) the j tiles [0, jt_end) read: up to the last tile's window end.
+int64_t x_cols_for_tiles(const dd_plan *plan, int jt_end)
+{
+    const dd::Tiling &t = plan->til;
+    if (jt_end >= t.ntj) return t.Lw;
+    const int64_t need = static_cast<int64_t>(jt_end) * t.shape.D_J() + plan->max_shift + 4;
+    const int64_t up = (need + 3) / 4 * 4;
+    return up < t.Lw ? up : t.Lw;
+}
+
+// Launch the pre-pass for X columns [x0, x1) and the main kernel for j tiles [jt0, jt1).
+int launch_range(const dd_plan *plan, const void *d_in, void *d_out, cudaStream_t st, int64_t x0,
+                 int64_t x1, int jt0, int jt1, const cudaEvent_t *ev)
+{
+    const dd::Tiling &t = plan->til;
+    if (ev) cudaEventRecord(ev[0], st);
+    if (x1 > x0) {
+        dd::InterleaveParams ip;
+        ip.in = d_in;
+        ip.X = plan->d_X;
+        ip.nsamps = plan->nsamps;
+        ip.L = t.L;
+        ip.Lw = t.Lw;
+        ip.nchans = plan->nchans;
+        ip.j_begin = x0;
+        ip.j_end = x1;
+        ip.nchunk = static_cast<int>((x1 - x0 + 1023) / 1024);
+        if (dd::launch_interleave(plan->in_dtype, t.shape.VW, ip, st) != 0) return DD_ERR_CUDA;
+    }
+    if (ev) cudaEventRecord(ev[1], st);
+    if (jt1 > jt0) {
+        dd::KernelParams kp;
+        kp.X = plan->d_X;
+        kp.ofs = plan->d_ofs;
+        kp.blk = plan->d_blk;
+        kp.out = d_out;
+        kp.out_len = plan->out_len;
+        kp.Lw = t.Lw;
+        kp.L = t.L;
+        kp.ndm = plan->ndm;
+        kp.nch_pad = t.nch_pad;
+        kp.nk = t.nk;
+        kp.ndb = t.ndb;
+        kp.ntj = t.ntj;
+        kp.jt_begin = jt0;
+        kp.rows_bytes = t.rows_bytes;
+        kp.nstage = t.nstage;
+        kp.stage_bytes = t.rows_bytes + t.shape.D_DM() * t.shape.CH * t.shape.OW;
+        kp.one = 1u;
+        const int grid = t.ndb * (jt1 - jt0);
+        if (dd::launch_dedisperse(t.variant, kp, grid, static_cast<int>(t.smem_bytes), st) != 0)
+            return DD_ERR_CUDA;
+    }
+    if (ev) cudaEventRecord(ev[2], st);
+    return DD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
 int dd_execute(const dd_plan *plan, const void *d_in, void *d_out, void *cuda_stream)
 {
     if (!plan || !d_in || !d_out) return DD_ERR_INVALID_ARG;
     const dd::Tiling &t = plan->til;
-    dd::InterleaveParams ip;
-    ip.in = d_in;
-    ip.X = plan->d_X;
-    ip.nsamps = plan->nsamps;
-    ip.L = t.L;
-    ip.Lw = t.Lw;
-    ip.nchans = plan->nchans;
-    ip.nchunk = static_cast<int>((t.Lw + 1023) / 1024);
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const cudaEvent_t *ev = plan->timing ? plan->ev[plan->timed_count % dd_plan::kRing] : nullptr;
-    if (ev) cudaEventRecord(ev[0], st);
-    if (dd::launch_interleave(plan->in_dtype, t.shape.VW, ip, cuda_stream) != 0) return DD_ERR_CUDA;
-    if (ev) cudaEventRecord(ev[1], st);
-
-    dd::KernelParams kp;
-    kp.X = plan->d_X;
-    kp.ofs = plan->d_ofs;
-    kp.blk = plan->d_blk;
-    kp.out = d_out;
-    kp.out_len = plan->out_len;
-    kp.Lw = t.Lw;
-    kp.L = t.L;
-    kp.ndm = plan->ndm;
-    kp.nch_pad = t.nch_pad;
-    kp.nk = t.nk;
-    kp.ndb = t.ndb;
-    kp.ntj = t.ntj;
-    kp.rows_bytes = t.rows_bytes;
-    kp.nstage = t.nstage;
-    kp.stage_bytes = t.rows_bytes + t.shape.D_DM() * t.shape.CH * t.shape.OW;
-    kp.one = 1u;
-    const int grid = t.ndb * t.ntj;
-    if (dd::launch_dedisperse(t.variant, kp, grid, static_cast<int>(t.smem_bytes), cuda_stream) != 0)
-        return DD_ERR_CUDA;
-    if (ev) {
-        cudaEventRecord(ev[2], st);
-        ++plan->timed_count;
-    }
-    return DD_OK;
+    const int rc = launch_range(plan, d_in, d_out, st, 0, t.Lw, 0, t.ntj, ev);
+    if (rc == DD_OK && ev) ++plan->timed_count;
+    return rc;
 }
 
 int dd_plan_set_timing(dd_plan *plan, int on)
@@ -262,10 +303,18 @@ int dd_plan_kernel_times(dd_plan *plan, int max_n, float *interleave_ms, float *
     return static_cast<int>(n);
 }
 
+// Host-buffer path, pipelined: the j tiles are cut into up to kHostChunks groups; group g's
+// input time ranges (one per lane of the interleaved layout, all channels: strided 2-D
+// copies) travel host->device on a copy stream while group g-1 is being interleaved and
+// dedispersed on the caller's stream and group g-2's output ranges travel device->host on
+// a second copy stream.  PCIe is full duplex, so the step costs about
+// max(H2D, kernels, D2H) plus one group of fill and drain instead of their sum.
 int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream)
 {
     if (!plan || !h_in || !h_out) return DD_ERR_INVALID_ARG;
-    const size_t in_bytes = static_cast<size_t>(plan->nchans) * plan->nsamps * elem_bytes(plan->in_dtype);
+    const dd::Tiling &t = plan->til;
+    const size_t eb = elem_bytes(plan->in_dtype);
+    const size_t in_bytes = static_cast<size_t>(plan->nchans) * plan->nsamps * eb;
     const size_t out_bytes = static_cast<size_t>(plan->ndm) * plan->out_len * 4;
     if (!plan->d_in_own && cudaMalloc(&plan->d_in_own, in_bytes) != cudaSuccess) {
         cudaGetLastError();
@@ -277,13 +326,70 @@ int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_str
         plan->d_out_own = nullptr;
         return DD_ERR_ALLOC;
     }
+    if (!plan->host_made) {
+        if (cudaStreamCreateWithFlags(&plan->st_h2d, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaStreamCreateWithFlags(&plan->st_d2h, cudaStreamNonBlocking) != cudaSuccess)
+            return DD_ERR_CUDA;
+        for (int g = 0; g <= dd_plan::kHostChunks; ++g)
+            if (cudaEventCreateWithFlags(&plan->ev_in[g], cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&plan->ev_done[g], cudaEventDisableTiming) != cudaSuccess)
+                return DD_ERR_CUDA;
+        plan->host_made = true;
+    }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    if (cudaMemcpyAsync(plan->d_in_own, h_in, in_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess)
-        return DD_ERR_CUDA;
-    const int rc = dd_execute(plan, plan->d_in_own, plan->d_out_own, cuda_stream);
-    if (rc != DD_OK) return rc;
-    if (cudaMemcpyAsync(h_out, plan->d_out_own, out_bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess)
-        return DD_ERR_CUDA;
+    const int G = t.ntj < dd_plan::kHostChunks ? t.ntj : dd_plan::kHostChunks;
+    const int NL = t.shape.lanes();
+    const int64_t DJ = t.shape.D_J();
+    const unsigned char *hin = static_cast<const unsigned char *>(h_in);
+    unsigned char *din = static_cast<unsigned char *>(plan->d_in_own);
+    unsigned char *hout = static_cast<unsigned char *>(h_out);
+    const unsigned char *dout = static_cast<const unsigned char *>(plan->d_out_own);
+    const size_t in_pitch = static_cast<size_t>(plan->nsamps) * eb;
+    const size_t out_pitch = static_cast<size_t>(plan->out_len) * 4;
+
+    // the copy stream starts after whatever the caller has queued on `st`
+    if (cudaEventRecord(plan->ev_done[G], st) != cudaSuccess) return DD_ERR_CUDA;
+    cudaStreamWaitEvent(plan->st_h2d, plan->ev_done[G], 0);
+    int64_t x0 = 0;
+    for (int g = 0; g < G; ++g) {
+        const int jt0 = static_cast<int>(static_cast<int64_t>(t.ntj) * g / G);
+        const int jt1 = static_cast<int>(static_cast<int64_t>(t.ntj) * (g + 1) / G);
+        const int64_t x1 = x_cols_for_tiles(plan, jt1);
+        // ---- host -> device: lane l needs times [l*L + x0, l*L + x1); what lies past
+        // (l+1)*L was already brought in by lane l+1's first group
+        for (int l = 0; l < NL; ++l) {
+            const int64_t lo = l * t.L + x0;
+            int64_t hi = l * t.L + x1;
+            if (l + 1 < NL && hi > (l + 1) * t.L) hi = (l + 1) * t.L;
+            if (hi > plan->nsamps) hi = plan->nsamps;
+            if (hi <= lo) continue;
+            if (cudaMemcpy2DAsync(din + lo * eb, in_pitch, hin + lo * eb, in_pitch,
+                                  static_cast<size_t>(hi - lo) * eb, plan->nchans,
+                                  cudaMemcpyHostToDevice, plan->st_h2d) != cudaSuccess)
+                return DD_ERR_CUDA;
+        }
+        cudaEventRecord(plan->ev_in[g], plan->st_h2d);
+        // ---- kernels for this group on the caller's stream
+        cudaStreamWaitEvent(st, plan->ev_in[g], 0);
+        const int rc = launch_range(plan, plan->d_in_own, plan->d_out_own, st, x0, x1, jt0, jt1, nullptr);
+        if (rc != DD_OK) return rc;
+        cudaEventRecord(plan->ev_done[g], st);
+        // ---- device -> host: output samples l*L + [jt0*D_J, jt1*D_J) of every DM row
+        cudaStreamWaitEvent(plan->st_d2h, plan->ev_done[g], 0);
+        const int64_t ja = jt0 * DJ, jb = jt1 * DJ < t.L ? jt1 * DJ : t.L;
+        for (int l = 0; l < NL; ++l) {
+            const int64_t lo = l * t.L + ja;
+            int64_t hi = l * t.L + jb;
+            if (hi > plan->out_len) hi = plan->out_len;
+            if (hi <= lo) continue;
+            if (cudaMemcpy2DAsync(hout + lo * 4, out_pitch, dout + lo * 4, out_pitch,
+                                  static_cast<size_t>(hi - lo) * 4, plan->ndm,
+                                  cudaMemcpyDeviceToHost, plan->st_d2h) != cudaSuccess)
+                return DD_ERR_CUDA;
+        }
+        x0 = x1;
+    }
+    if (cudaStreamSynchronize(plan->st_d2h) != cudaSuccess) return DD_ERR_CUDA;
     if (cudaStreamSynchronize(st) != cudaSuccess) return DD_ERR_CUDA;
     return DD_OK;
 }

@@ -74,6 +74,7 @@ struct KernelParams {
     int64_t Lw;        // superwords per row of X
     int64_t L;
     int ndm, nch_pad, nk, ndb, ntj;
+    int jt_begin;      // first j tile of this launch (the grid covers a range of tiles)
     int rows_bytes;    // channel windows of one stage; the stage's offset table follows
     int nstage;
     int stage_bytes;   // rows_bytes + D_DM*CH*OW, multiple of 16
@@ -85,7 +86,8 @@ struct InterleaveParams {
     uint32_t *X;
     int64_t nsamps, L, Lw;
     int nchans;
-    int nchunk;  // blocks per channel row: ceil(Lw / (4 * 256)), a thread makes 4 superwords
+    int64_t j_begin, j_end;  // superword columns [j_begin, j_end) of X to fill (multiples of 4)
+    int nchunk;  // blocks per channel row: ceil((j_end - j_begin) / (4 * 256)), a thread makes 4 superwords
 };
 
 int num_variants();

@@ -209,7 +209,7 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int b = blockIdx.x % p.ndb;  // DM block fastest: co-resident blocks share input
-    const int jt = blockIdx.x / p.ndb;
+    const int jt = blockIdx.x / p.ndb + p.jt_begin;
     const int64_t j0 = static_cast<int64_t>(jt) * D_J;
     const int nstage = p.nstage;
 
@@ -374,8 +374,8 @@ template <int MODE, int VW>
 __global__ void __launch_bounds__(256) interleave_kernel(const InterleaveParams p)
 {
     const int c = static_cast<int>(blockIdx.x / p.nchunk);
-    const int64_t j = (static_cast<int64_t>(blockIdx.x % p.nchunk) * blockDim.x + threadIdx.x) * 4;
-    if (j >= p.Lw) return;
+    const int64_t j = p.j_begin + (static_cast<int64_t>(blockIdx.x % p.nchunk) * blockDim.x + threadIdx.x) * 4;
+    if (j >= p.j_end) return;
     uint32_t w[4 * VW];  // w[q * VW + v] = word v of superword j + q
     if (MODE == DD_U8) {
         const uint8_t *row = static_cast<const uint8_t *>(p.in) + static_cast<size_t>(c) * p.nsamps;

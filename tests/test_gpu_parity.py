@@ -269,6 +269,34 @@ def test_repeat_execute_streams_and_host_path(B, oracle):
     plan.destroy()
 
 
+@pytest.mark.parametrize("dtype", [np.uint8, np.uint16, np.float32])
+@pytest.mark.parametrize("case", CASES)
+def test_host_path_pipelined_chunks_match_oracle(B, oracle, dtype, case):
+    """dd_execute_host cuts the j tiles into groups and moves per-lane time ranges with
+    strided copies; pageable and sentinel-filled buffers, ragged sizes, every dtype."""
+    import torch
+    nchans, nsamps, ndm, step, f_high, band, tsamp = case
+    rng = np.random.default_rng([nchans, nsamps, ndm, 5])
+    x = _rand_input(rng, dtype, nchans, nsamps)
+    dms = np.arange(ndm) * step
+    plan = B.Plan(nchans, nsamps, f_high, -band / nchans, tsamp, dms,
+                  {np.uint8: B.DD_U8, np.uint16: B.DD_U16, np.float32: B.DD_F32}[dtype])
+    try:
+        xt = torch.from_numpy(x.view(np.int16) if dtype == np.uint16 else x)
+        odt = torch.float32 if dtype == np.float32 else torch.int32
+        for pinned in (True, False):
+            h_in = xt.pin_memory() if pinned else xt
+            h_out = torch.full((plan.ndm, plan.out_len), -7, dtype=odt)
+            if pinned:
+                h_out = h_out.pin_memory()
+            plan.execute_host(h_in, h_out)
+            got = h_out.numpy()
+            check_against_oracle(oracle, x, got if dtype == np.float32 else got.view(np.uint32),
+                                 plan.shift_table(), plan.out_len)
+    finally:
+        plan.destroy()
+
+
 def test_plan_errors_on_gpu(B):
     with pytest.raises(B.DDError) as e:
         B.Plan(4, 32, 1500.0, -25.0, 1e-3, [0.0, 300.0], B.DD_U8)
