@@ -181,7 +181,7 @@ def _config_dict(cfg, plan):
         d.update({"out_len": plan.out_len, "max_shift": plan.max_shift,
                   "adds_per_step": plan.ndm * plan.out_len * cfg.nchans,
                   "adds_nominal": cfg.ndm * cfg.nsamps * cfg.nchans,
-                  "tile": "D_DM=%d x D_J=%d words x %d lanes, CH=%d, %d stages, %d B smem, grid %d x %d threads"
+                  "tile": "D_DM=%d x D_J=%d superwords x %d lanes, CH=%d, %d stages, %d B smem, grid %d x %d threads"
                           % (plan.info("D_DM"), plan.info("D_J"), plan.info("LANES"), plan.info("CH"),
                              plan.info("NSTAGE"), plan.info("SMEM_BYTES"), plan.info("GRID"),
                              plan.info("THREADS"))})
@@ -285,19 +285,29 @@ def run_ours(args):
     in_b = W.ELEM_BYTES[cfg.in_dtype]
     smem_alg_bytes = adds * in_b                      # one sample read from shared memory per add
     hbm_alg_bytes = cfg.nchans * cfg.nsamps * in_b + plan.ndm * plan.out_len * 4
-    roofline = {"bound": "alu", "kernel": "dedisperse_kernel",
-                "achieved": kadds / 1e12, "peak": int_peak / 1e12, "unit": "Tadd/s",
-                "frac": kadds / int_peak, "traffic": None,
-                "peak_kind": "derived: %d SMs x %d INT32 add lanes/clk x %.0f MHz (%s sm_max_mhz)"
-                             % (N_SM, INT_LANES_PER_SM_CLK, sm_max_mhz, peak_kind),
-                "note": "achieved counts sample-adds; one packed IADD3 lane-instruction performs up "
-                        "to 4 (u8) / 2 (u16) sample-adds, so frac may exceed 1",
-                "kernel_ms": main_s * 1e3, "share_of_step": main_s / (main_s + il_s)}
-    roofline_smem = {"bound": "smem", "achieved": smem_alg_bytes / main_s / 1e9, "peak": smem_peak_gbs,
-                     "unit": "GB/s", "frac": smem_alg_bytes / main_s / 1e9 / smem_peak_gbs,
-                     "peak_kind": "derived (paper Eq. 8): %d SMs x %d B/clk x %.0f MHz"
-                                  % (N_SM, SMEM_BYTES_PER_SM_CLK, sm_max_mhz),
-                     "bytes_per_add": in_b}
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "r01b_traffic.json")
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            traffic = json.load(f).get(cfg.name)
+    share = main_s / (main_s + il_s)
+    # The dominant kernel reads one sample from shared memory per add: its binding roofline is the
+    # shared-memory pipe (ncu: 90-99 % of peak wavefronts), reported in bytes.
+    roofline = {"bound": "smem", "kernel": "dedisperse_kernel",
+                "achieved": smem_alg_bytes / main_s / 1e9, "peak": smem_peak_gbs, "unit": "GB/s",
+                "frac": smem_alg_bytes / main_s / 1e9 / smem_peak_gbs, "traffic": traffic,
+                "traffic_note": "DRAM bytes per launch (ncu, profiles/r01b_summary.md); algorithmic HBM bytes %d"
+                                % hbm_alg_bytes,
+                "peak_kind": "derived (paper Eq. 8): %d SMs x %d B/clk x %.0f MHz (%s sm_max_mhz)"
+                             % (N_SM, SMEM_BYTES_PER_SM_CLK, sm_max_mhz, peak_kind),
+                "algorithmic_bytes_per_add": in_b, "adds_per_launch": adds,
+                "kernel_ms": main_s * 1e3, "share_of_step": share}
+    roofline_alu = {"bound": "alu", "achieved": kadds / 1e12, "peak": int_peak / 1e12, "unit": "Tadd/s",
+                    "frac": kadds / int_peak,
+                    "peak_kind": "derived: %d SMs x %d INT32 add lanes/clk x %.0f MHz"
+                                 % (N_SM, INT_LANES_PER_SM_CLK, sm_max_mhz),
+                    "note": "sample-adds against one-add-per-lane integer peak (BASELINE.json's metric); "
+                            "a packed add performs 4 (u8) / 2 (u16) sample-adds, so frac may exceed 1"}
     roofline_hbm = {"bound": "hbm", "achieved": hbm_alg_bytes / (ms_step * 1e-3) / 1e9, "peak": hbm_gbs,
                     "unit": "GB/s", "frac": hbm_alg_bytes / (ms_step * 1e-3) / 1e9 / hbm_gbs,
                     "peak_kind": peak_kind + " copy bandwidth",
@@ -313,7 +323,7 @@ def run_ours(args):
                                 "out_len_tsamp_over_t": plan.out_len * cfg.tsamp / (ms_step * 1e-3)},
             "value_nominal": world * cfg.ndm * cfg.nsamps * cfg.nchans / (ms_step * 1e-3),
             "kernels_ms": {"interleave_kernel": il_s * 1e3, "dedisperse_kernel": main_s * 1e3},
-            "roofline": roofline, "roofline_smem": roofline_smem, "roofline_hbm": roofline_hbm,
+            "roofline": roofline, "roofline_alu": roofline_alu, "roofline_hbm": roofline_hbm,
             "cpu_baseline": cpu_base,
             "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e,
                     "steps": e2e_steps, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,

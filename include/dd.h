@@ -97,10 +97,14 @@ int dd_execute(const dd_plan *plan, const void *d_in, void *d_out, void *cuda_st
 
 /*
  * The same transform with HOST buffers: h_in [nchans][nsamps], h_out [ndm][out_len].
- * Copies h_in to a plan-owned device buffer, runs dd_execute, copies the result back and
- * waits for the stream.  Buffers should be page-locked for full PCIe bandwidth (pageable
- * memory works, slower).  The device buffers are allocated on first use and kept until
- * dd_plan_destroy.  Errors as dd_execute, plus DD_ERR_ALLOC.
+ * Pipelined over up to 8 time chunks (default 6; environment variable DD_HOST_CHUNKS=<n>
+ * overrides): chunk g's input range [o0, o1 + max_shift) of every channel is copied to a
+ * plan-owned device buffer on a copy stream while chunk g-1 runs through the kernels on
+ * `cuda_stream` and chunk g-2's output columns are copied back on a second copy stream.
+ * Returns after the last copy has finished.  Buffers should be page-locked for full PCIe
+ * bandwidth and true overlap (pageable memory works, slower).  The device buffers, two
+ * streams and the events are created on first use and kept until dd_plan_destroy.
+ * Errors as dd_execute, plus DD_ERR_ALLOC.
  */
 int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream);
 

@@ -198,59 +198,70 @@ int dd_plan_shift_table(const dd_plan *plan, const int32_t **table, int64_t *out
 
 namespace {
 
-// X columns (superwords) the j tiles [0, jt_end) read: up to the last tile's window end.
-int64_t x_cols_for_tiles(const dd_plan *plan, int jt_end)
+// One launch pair over a block of `nsamps` input samples per channel producing `out_len`
+// output samples per DM trial: the whole plan (dd_execute) or one time chunk of it
+// (dd_execute_host).  The tiling tables do not depend on the block length, only L, the
+// number of j tiles and the workspace row length do.
+struct BlockGeom {
+    int64_t nsamps, out_len;  // valid input / output samples of this block
+    int64_t L, Lw;
+    int ntj;
+};
+
+BlockGeom geom_for(const dd_plan *plan, int64_t out_len, int64_t nsamps)
 {
     const dd::Tiling &t = plan->til;
-    if (jt_end >= t.ntj) return t.Lw;
-    const int64_t need = static_cast<int64_t>(jt_end) * t.shape.D_J() + plan->max_shift + 4;
-    const int64_t up = (need + 3) / 4 * 4;
-    return up < t.Lw ? up : t.Lw;
+    BlockGeom g;
+    g.nsamps = nsamps;
+    g.out_len = out_len;
+    const int NL = t.shape.lanes();
+    g.L = ((out_len + NL - 1) / NL + 15) / 16 * 16;
+    g.ntj = static_cast<int>((g.L + t.shape.D_J() - 1) / t.shape.D_J());
+    g.Lw = (static_cast<int64_t>(g.ntj) * t.shape.D_J() + plan->max_shift + 4 + 3) / 4 * 4;
+    return g;
 }
 
-// Launch the pre-pass for X columns [x0, x1) and the main kernel for j tiles [jt0, jt1).
-int launch_range(const dd_plan *plan, const void *d_in, void *d_out, cudaStream_t st, int64_t x0,
-                 int64_t x1, int jt0, int jt1, const cudaEvent_t *ev)
+int launch_block(const dd_plan *plan, const BlockGeom &g, const void *d_in, int64_t in_pitch,
+                 void *d_out, int64_t out_pitch, cudaStream_t st, const cudaEvent_t *ev)
 {
     const dd::Tiling &t = plan->til;
     if (ev) cudaEventRecord(ev[0], st);
-    if (x1 > x0) {
-        dd::InterleaveParams ip;
-        ip.in = d_in;
-        ip.X = plan->d_X;
-        ip.nsamps = plan->nsamps;
-        ip.L = t.L;
-        ip.Lw = t.Lw;
-        ip.nchans = plan->nchans;
-        ip.j_begin = x0;
-        ip.j_end = x1;
-        ip.nchunk = static_cast<int>((x1 - x0 + 1023) / 1024);
-        if (dd::launch_interleave(plan->in_dtype, t.shape.VW, ip, st) != 0) return DD_ERR_CUDA;
-    }
+    dd::InterleaveParams ip;
+    ip.in = d_in;
+    ip.X = plan->d_X;
+    ip.nsamps = g.nsamps;
+    ip.in_pitch = in_pitch;
+    ip.L = g.L;
+    ip.Lw = g.Lw;
+    ip.nchans = plan->nchans;
+    ip.nrows = t.nch_pad;
+    ip.j_begin = 0;
+    ip.j_end = g.Lw;
+    ip.nchunk = static_cast<int>((g.Lw + 1023) / 1024);
+    if (dd::launch_interleave(plan->in_dtype, t.shape.VW, ip, st) != 0) return DD_ERR_CUDA;
     if (ev) cudaEventRecord(ev[1], st);
-    if (jt1 > jt0) {
-        dd::KernelParams kp;
-        kp.X = plan->d_X;
-        kp.ofs = plan->d_ofs;
-        kp.blk = plan->d_blk;
-        kp.out = d_out;
-        kp.out_len = plan->out_len;
-        kp.Lw = t.Lw;
-        kp.L = t.L;
-        kp.ndm = plan->ndm;
-        kp.nch_pad = t.nch_pad;
-        kp.nk = t.nk;
-        kp.ndb = t.ndb;
-        kp.ntj = t.ntj;
-        kp.jt_begin = jt0;
-        kp.rows_bytes = t.rows_bytes;
-        kp.nstage = t.nstage;
-        kp.stage_bytes = t.rows_bytes + t.shape.D_DM() * t.shape.CH * t.shape.OW;
-        kp.one = 1u;
-        const int grid = t.ndb * (jt1 - jt0);
-        if (dd::launch_dedisperse(t.variant, kp, grid, static_cast<int>(t.smem_bytes), st) != 0)
-            return DD_ERR_CUDA;
-    }
+    dd::KernelParams kp;
+    kp.X = plan->d_X;
+    kp.ofs = plan->d_ofs;
+    kp.blk = plan->d_blk;
+    kp.out = d_out;
+    kp.out_len = g.out_len;
+    kp.out_pitch = out_pitch;
+    kp.Lw = g.Lw;
+    kp.L = g.L;
+    kp.ndm = plan->ndm;
+    kp.nch_pad = t.nch_pad;
+    kp.nk = t.nk;
+    kp.ndb = t.ndb;
+    kp.ntj = g.ntj;
+    kp.jt_begin = 0;
+    kp.rows_bytes = t.rows_bytes;
+    kp.nstage = t.nstage;
+    kp.stage_bytes = t.rows_bytes + t.shape.D_DM() * t.shape.CH * t.shape.OW;
+    kp.one = 1u;
+    const int grid = t.ndb * g.ntj;
+    if (dd::launch_dedisperse(t.variant, kp, grid, static_cast<int>(t.smem_bytes), st) != 0)
+        return DD_ERR_CUDA;
     if (ev) cudaEventRecord(ev[2], st);
     return DD_OK;
 }
@@ -262,10 +273,10 @@ extern "C" {
 int dd_execute(const dd_plan *plan, const void *d_in, void *d_out, void *cuda_stream)
 {
     if (!plan || !d_in || !d_out) return DD_ERR_INVALID_ARG;
-    const dd::Tiling &t = plan->til;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const cudaEvent_t *ev = plan->timing ? plan->ev[plan->timed_count % dd_plan::kRing] : nullptr;
-    const int rc = launch_range(plan, d_in, d_out, st, 0, t.Lw, 0, t.ntj, ev);
+    const BlockGeom g = geom_for(plan, plan->out_len, plan->nsamps);
+    const int rc = launch_block(plan, g, d_in, plan->nsamps, d_out, plan->out_len, st, ev);
     if (rc == DD_OK && ev) ++plan->timed_count;
     return rc;
 }
@@ -303,12 +314,14 @@ int dd_plan_kernel_times(dd_plan *plan, int max_n, float *interleave_ms, float *
     return static_cast<int>(n);
 }
 
-// Host-buffer path, pipelined: the j tiles are cut into up to kHostChunks groups; group g's
-// input time ranges (one per lane of the interleaved layout, all channels: strided 2-D
-// copies) travel host->device on a copy stream while group g-1 is being interleaved and
-// dedispersed on the caller's stream and group g-2's output ranges travel device->host on
-// a second copy stream.  PCIe is full duplex, so the step costs about
-// max(H2D, kernels, D2H) plus one group of fill and drain instead of their sum.
+// Host-buffer path, pipelined over TIME CHUNKS (the time sharding of SURVEY.md 8(e) applied
+// inside one GPU): chunk g produces output samples [o0, o1) of every DM trial from input
+// samples [o0, o1 + max_shift) of every channel.  Its new input samples travel host->device
+// on a copy stream (one strided 2-D copy: all channels x a contiguous time range) while
+// chunk g-1 is interleaved and dedispersed on the caller's stream and chunk g-2's output
+// columns travel device->host on a second copy stream.  PCIe is full duplex, so a step costs
+// about max(H2D, kernels, D2H) plus one chunk of fill and drain instead of their sum.  The
+// kernels see a chunk as a smaller block of the same plan (same shift and tiling tables).
 int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream)
 {
     if (!plan || !h_in || !h_out) return DD_ERR_INVALID_ARG;
@@ -337,57 +350,56 @@ int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_str
         plan->host_made = true;
     }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    const int G = t.ntj < dd_plan::kHostChunks ? t.ntj : dd_plan::kHostChunks;
+    // chunk length: a multiple of 16 samples per lane (keeps every chunk's rows as aligned as the
+    // caller's), at least 8 j tiles per chunk so that the grid still fills the GPU
     const int NL = t.shape.lanes();
-    const int64_t DJ = t.shape.D_J();
+    const int64_t tile = static_cast<int64_t>(NL) * t.shape.D_J();
+    int want = 6;  // measured best on the headline config (profiles/r01_tuning.md)
+    if (const char *e = std::getenv("DD_HOST_CHUNKS")) {  // explicit request (tests, tuning)
+        want = std::atoi(e);
+    } else {
+        const int64_t by_tiles = plan->out_len / (8 * tile);
+        if (want > by_tiles) want = static_cast<int>(by_tiles);
+    }
+    if (want > dd_plan::kHostChunks) want = dd_plan::kHostChunks;
+    if (want < 1) want = 1;
+    const int64_t unit = static_cast<int64_t>(NL) * 16;
+    const int64_t C = ((plan->out_len + want - 1) / want + unit - 1) / unit * unit;
+    const int G = static_cast<int>((plan->out_len + C - 1) / C);
+
     const unsigned char *hin = static_cast<const unsigned char *>(h_in);
     unsigned char *din = static_cast<unsigned char *>(plan->d_in_own);
     unsigned char *hout = static_cast<unsigned char *>(h_out);
-    const unsigned char *dout = static_cast<const unsigned char *>(plan->d_out_own);
+    unsigned char *dout = static_cast<unsigned char *>(plan->d_out_own);
     const size_t in_pitch = static_cast<size_t>(plan->nsamps) * eb;
     const size_t out_pitch = static_cast<size_t>(plan->out_len) * 4;
 
     // the copy stream starts after whatever the caller has queued on `st`
     if (cudaEventRecord(plan->ev_done[G], st) != cudaSuccess) return DD_ERR_CUDA;
     cudaStreamWaitEvent(plan->st_h2d, plan->ev_done[G], 0);
-    int64_t x0 = 0;
+    int64_t have = 0;  // input samples [0, have) of every channel are on their way to the device
     for (int g = 0; g < G; ++g) {
-        const int jt0 = static_cast<int>(static_cast<int64_t>(t.ntj) * g / G);
-        const int jt1 = static_cast<int>(static_cast<int64_t>(t.ntj) * (g + 1) / G);
-        const int64_t x1 = x_cols_for_tiles(plan, jt1);
-        // ---- host -> device: lane l needs times [l*L + x0, l*L + x1); what lies past
-        // (l+1)*L was already brought in by lane l+1's first group
-        for (int l = 0; l < NL; ++l) {
-            const int64_t lo = l * t.L + x0;
-            int64_t hi = l * t.L + x1;
-            if (l + 1 < NL && hi > (l + 1) * t.L) hi = (l + 1) * t.L;
-            if (hi > plan->nsamps) hi = plan->nsamps;
-            if (hi <= lo) continue;
-            if (cudaMemcpy2DAsync(din + lo * eb, in_pitch, hin + lo * eb, in_pitch,
-                                  static_cast<size_t>(hi - lo) * eb, plan->nchans,
+        const int64_t o0 = g * C, o1 = o0 + C < plan->out_len ? o0 + C : plan->out_len;
+        const int64_t need = o1 + plan->max_shift;  // <= nsamps
+        if (need > have) {
+            if (cudaMemcpy2DAsync(din + have * eb, in_pitch, hin + have * eb, in_pitch,
+                                  static_cast<size_t>(need - have) * eb, plan->nchans,
                                   cudaMemcpyHostToDevice, plan->st_h2d) != cudaSuccess)
                 return DD_ERR_CUDA;
+            have = need;
         }
         cudaEventRecord(plan->ev_in[g], plan->st_h2d);
-        // ---- kernels for this group on the caller's stream
         cudaStreamWaitEvent(st, plan->ev_in[g], 0);
-        const int rc = launch_range(plan, plan->d_in_own, plan->d_out_own, st, x0, x1, jt0, jt1, nullptr);
+        const BlockGeom bg = geom_for(plan, o1 - o0, need - o0);
+        const int rc = launch_block(plan, bg, din + o0 * eb, plan->nsamps, dout + o0 * 4,
+                                    plan->out_len, st, nullptr);
         if (rc != DD_OK) return rc;
         cudaEventRecord(plan->ev_done[g], st);
-        // ---- device -> host: output samples l*L + [jt0*D_J, jt1*D_J) of every DM row
         cudaStreamWaitEvent(plan->st_d2h, plan->ev_done[g], 0);
-        const int64_t ja = jt0 * DJ, jb = jt1 * DJ < t.L ? jt1 * DJ : t.L;
-        for (int l = 0; l < NL; ++l) {
-            const int64_t lo = l * t.L + ja;
-            int64_t hi = l * t.L + jb;
-            if (hi > plan->out_len) hi = plan->out_len;
-            if (hi <= lo) continue;
-            if (cudaMemcpy2DAsync(hout + lo * 4, out_pitch, dout + lo * 4, out_pitch,
-                                  static_cast<size_t>(hi - lo) * 4, plan->ndm,
-                                  cudaMemcpyDeviceToHost, plan->st_d2h) != cudaSuccess)
-                return DD_ERR_CUDA;
-        }
-        x0 = x1;
+        if (cudaMemcpy2DAsync(hout + o0 * 4, out_pitch, dout + o0 * 4, out_pitch,
+                              static_cast<size_t>(o1 - o0) * 4, plan->ndm, cudaMemcpyDeviceToHost,
+                              plan->st_d2h) != cudaSuccess)
+            return DD_ERR_CUDA;
     }
     if (cudaStreamSynchronize(plan->st_d2h) != cudaSuccess) return DD_ERR_CUDA;
     if (cudaStreamSynchronize(st) != cudaSuccess) return DD_ERR_CUDA;

@@ -70,7 +70,8 @@ struct KernelParams {
     const void *ofs;      // [ndb][nk][D_DM][CH] entries of OW bytes
     const int32_t *blk;   // 4 ints per slot (read as int4)
     void *out;
-    int64_t out_len;
+    int64_t out_len;   // valid output samples per DM row (stores are bounded by it)
+    int64_t out_pitch; // elements between consecutive DM rows of `out`
     int64_t Lw;        // superwords per row of X
     int64_t L;
     int ndm, nch_pad, nk, ndb, ntj;
@@ -84,8 +85,11 @@ struct KernelParams {
 struct InterleaveParams {
     const void *in;
     uint32_t *X;
-    int64_t nsamps, L, Lw;
-    int nchans;
+    int64_t nsamps;    // valid samples per channel row (reads past it give 0)
+    int64_t in_pitch;  // elements between consecutive channel rows of `in`
+    int64_t L, Lw;
+    int nchans;        // rows nchans .. nrows-1 of X are zero-filled (padding channels)
+    int nrows;
     int64_t j_begin, j_end;  // superword columns [j_begin, j_end) of X to fill (multiples of 4)
     int nchunk;  // blocks per channel row: ceil((j_end - j_begin) / (4 * 256)), a thread makes 4 superwords
 };

@@ -349,7 +349,7 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
                 } else {
                     val[0] = __float_as_uint(acc[r][i][v].s);
                 }
-                uint32_t *o = static_cast<uint32_t *>(p.out) + static_cast<size_t>(d) * p.out_len;
+                uint32_t *o = static_cast<uint32_t *>(p.out) + static_cast<size_t>(d) * p.out_pitch;
 #pragma unroll
                 for (int l = 0; l < LPW; ++l) {
                     const int64_t t = static_cast<int64_t>(v * LPW + l) * p.L + j;
@@ -377,8 +377,11 @@ __global__ void __launch_bounds__(256) interleave_kernel(const InterleaveParams 
     const int64_t j = p.j_begin + (static_cast<int64_t>(blockIdx.x % p.nchunk) * blockDim.x + threadIdx.x) * 4;
     if (j >= p.j_end) return;
     uint32_t w[4 * VW];  // w[q * VW + v] = word v of superword j + q
-    if (MODE == DD_U8) {
-        const uint8_t *row = static_cast<const uint8_t *>(p.in) + static_cast<size_t>(c) * p.nsamps;
+    if (c >= p.nchans) {  // padding channel (nchans rounded up to CH): a zero row
+#pragma unroll
+        for (int i = 0; i < 4 * VW; ++i) w[i] = 0u;
+    } else if (MODE == DD_U8) {
+        const uint8_t *row = static_cast<const uint8_t *>(p.in) + static_cast<size_t>(c) * p.in_pitch;
         const bool aligned = (reinterpret_cast<uintptr_t>(row) & 3u) == 0;
 #pragma unroll
         for (int v = 0; v < VW; ++v) {
@@ -405,7 +408,7 @@ __global__ void __launch_bounds__(256) interleave_kernel(const InterleaveParams 
             w[3 * VW + v] = __byte_perm(t01h, t23h, 0x7632);
         }
     } else if (MODE == DD_U16) {
-        const uint16_t *row = static_cast<const uint16_t *>(p.in) + static_cast<size_t>(c) * p.nsamps;
+        const uint16_t *row = static_cast<const uint16_t *>(p.in) + static_cast<size_t>(c) * p.in_pitch;
         const bool aligned = (reinterpret_cast<uintptr_t>(row) & 7u) == 0;
 #pragma unroll
         for (int v = 0; v < VW; ++v) {
@@ -426,7 +429,7 @@ __global__ void __launch_bounds__(256) interleave_kernel(const InterleaveParams 
             w[3 * VW + v] = __byte_perm(seg[0].y, seg[1].y, 0x7632);
         }
     } else {
-        const uint32_t *row = static_cast<const uint32_t *>(p.in) + static_cast<size_t>(c) * p.nsamps;
+        const uint32_t *row = static_cast<const uint32_t *>(p.in) + static_cast<size_t>(c) * p.in_pitch;
         const bool aligned = (reinterpret_cast<uintptr_t>(row) & 15u) == 0;
 #pragma unroll
         for (int v = 0; v < VW; ++v) {
@@ -526,7 +529,7 @@ static void launch_interleave_vw(int mode, const InterleaveParams &p, unsigned g
 
 int launch_interleave(int mode, int VW, const InterleaveParams &p, void *stream)
 {
-    const unsigned grid = static_cast<unsigned>(static_cast<int64_t>(p.nchunk) * p.nchans);
+    const unsigned grid = static_cast<unsigned>(static_cast<int64_t>(p.nchunk) * p.nrows);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if (VW == 1)
         launch_interleave_vw<1>(mode, p, grid, st);

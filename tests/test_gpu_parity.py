@@ -271,10 +271,12 @@ def test_repeat_execute_streams_and_host_path(B, oracle):
 
 @pytest.mark.parametrize("dtype", [np.uint8, np.uint16, np.float32])
 @pytest.mark.parametrize("case", CASES)
-def test_host_path_pipelined_chunks_match_oracle(B, oracle, dtype, case):
-    """dd_execute_host cuts the j tiles into groups and moves per-lane time ranges with
-    strided copies; pageable and sentinel-filled buffers, ragged sizes, every dtype."""
+def test_host_path_pipelined_chunks_match_oracle(B, oracle, dtype, case, monkeypatch):
+    """dd_execute_host cuts the output into time chunks (input range = chunk + max_shift halo,
+    strided 2-D copies on copy streams); 3 chunks forced here, pinned and pageable buffers,
+    sentinel-filled output, ragged sizes, every dtype."""
     import torch
+    monkeypatch.setenv("DD_HOST_CHUNKS", "3")
     nchans, nsamps, ndm, step, f_high, band, tsamp = case
     rng = np.random.default_rng([nchans, nsamps, ndm, 5])
     x = _rand_input(rng, dtype, nchans, nsamps)
