@@ -96,6 +96,19 @@ int dd_plan_shift_table(const dd_plan *plan, const int32_t **table, int64_t *out
 int dd_execute(const dd_plan *plan, const void *d_in, void *d_out, void *cuda_stream);
 
 /*
+ * The transform on TIME-MAJOR input, the order telescopes and SIGPROC filterbank files use:
+ *   d_in_tm: DEVICE, dense [nsamps][nchans] of the plan's in_dtype (channel 0 = f_high).
+ * A transpose kernel writes the channel-major block Eq. 3 / Alg. 3 index
+ * into a plan-owned device buffer (allocated on first use), then dd_execute runs on it; the
+ * paper counts this transpose in its pipeline time.  Same stream semantics,
+ * output and errors as dd_execute, plus DD_ERR_ALLOC.  With timing on
+ * (dd_plan_set_timing), dd_plan_transpose_time returns the duration in milliseconds of
+ * the latest timed call's transpose kernel (DD_ERR_INVALID_ARG if there is none).
+ */
+int dd_execute_tm(dd_plan *plan, const void *d_in_tm, void *d_out, void *cuda_stream);
+int dd_plan_transpose_time(dd_plan *plan, float *ms);
+
+/*
  * The same transform with HOST buffers: h_in [nchans][nsamps], h_out [ndm][out_len].
  * Pipelined over up to 8 time chunks (default 6; environment variable DD_HOST_CHUNKS=<n>
  * overrides): chunk g's input range [o0, o1 + max_shift) of every channel is copied to a

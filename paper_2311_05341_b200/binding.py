@@ -28,7 +28,7 @@ INFO = {"D_DM": 0, "D_J": 1, "LANES": 2, "L": 3, "SMEM_BYTES": 4, "GRID": 5, "TH
 
 # every symbol include/dd.h declares (tests check the .so exports all of them)
 SYMBOLS = ("dd_shift_table_build", "dd_plan_create", "dd_plan_shift_table", "dd_execute",
-           "dd_execute_host", "dd_plan_info", "dd_plan_set_timing", "dd_plan_kernel_times",
+           "dd_execute_host", "dd_execute_tm", "dd_plan_transpose_time", "dd_plan_info", "dd_plan_set_timing", "dd_plan_kernel_times",
            "dd_plan_destroy", "dd_strerror", "dd_version")
 
 _lib = None
@@ -62,6 +62,10 @@ def lib() -> ctypes.CDLL:
         L.dd_execute.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p]
         L.dd_execute_host.restype = c.c_int
         L.dd_execute_host.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p]
+        L.dd_execute_tm.restype = c.c_int
+        L.dd_execute_tm.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p]
+        L.dd_plan_transpose_time.restype = c.c_int
+        L.dd_plan_transpose_time.argtypes = [c.c_void_p, c.POINTER(c.c_float)]
         L.dd_plan_info.restype = c.c_int64
         L.dd_plan_info.argtypes = [c.c_void_p, c.c_int]
         L.dd_plan_set_timing.restype = c.c_int
@@ -143,6 +147,20 @@ class Plan:
         rc = lib().dd_execute(self._h, _dev_ptr(d_in), _dev_ptr(d_out), _stream_ptr(stream))
         if rc != DD_OK:
             raise DDError(rc, "dd_execute")
+
+    # -- dd_execute_tm / dd_plan_transpose_time
+    def execute_tm(self, d_in_tm, d_out, stream=None) -> None:
+        """d_in_tm: time-major [nsamps][nchans] torch CUDA tensor (dense) or raw device address."""
+        rc = lib().dd_execute_tm(self._h, _dev_ptr(d_in_tm), _dev_ptr(d_out), _stream_ptr(stream))
+        if rc != DD_OK:
+            raise DDError(rc, "dd_execute_tm")
+
+    def transpose_time(self) -> float:
+        ms = ctypes.c_float(0.0)
+        rc = lib().dd_plan_transpose_time(self._h, ctypes.byref(ms))
+        if rc != DD_OK:
+            raise DDError(rc, "dd_plan_transpose_time")
+        return float(ms.value)
 
     # -- dd_execute_host
     def execute_host(self, h_in, h_out, stream=None) -> None:

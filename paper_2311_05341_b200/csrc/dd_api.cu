@@ -34,6 +34,8 @@ struct dd_plan {
     cudaEvent_t ev[kRing][3] = {};
     bool ev_made = false;
     mutable int64_t timed_count = 0;
+    cudaEvent_t ev_tm[2] = {};  // around the transpose of the latest timed dd_execute_tm
+    bool tm_timed = false;
 };
 
 namespace {
@@ -55,6 +57,8 @@ void free_device(dd_plan *p)
         if (p->ev_made)
             for (auto &triple : p->ev)
                 for (cudaEvent_t e : triple) cudaEventDestroy(e);
+        for (cudaEvent_t e : p->ev_tm)
+            if (e) cudaEventDestroy(e);
         if (p->host_made) {
             for (cudaEvent_t e : p->ev_in) cudaEventDestroy(e);
             for (cudaEvent_t e : p->ev_done) cudaEventDestroy(e);
@@ -281,6 +285,47 @@ int dd_execute(const dd_plan *plan, const void *d_in, void *d_out, void *cuda_st
     return rc;
 }
 
+int dd_execute_tm(dd_plan *plan, const void *d_in_tm, void *d_out, void *cuda_stream)
+{
+    if (!plan || !d_in_tm || !d_out) return DD_ERR_INVALID_ARG;
+    const size_t in_bytes = static_cast<size_t>(plan->nchans) * plan->nsamps * elem_bytes(plan->in_dtype);
+    if (!plan->d_in_own && cudaMalloc(&plan->d_in_own, in_bytes) != cudaSuccess) {
+        cudaGetLastError();
+        plan->d_in_own = nullptr;
+        return DD_ERR_ALLOC;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    dd::TransposeParams tp;
+    tp.in = d_in_tm;
+    tp.out = plan->d_in_own;
+    tp.nsamps = plan->nsamps;
+    tp.nchans = plan->nchans;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (plan->timing) {
+        if (!plan->ev_tm[0] && (cudaEventCreate(&plan->ev_tm[0]) != cudaSuccess ||
+                                cudaEventCreate(&plan->ev_tm[1]) != cudaSuccess))
+            return DD_ERR_CUDA;
+        e0 = plan->ev_tm[0];
+        e1 = plan->ev_tm[1];
+        cudaEventRecord(e0, st);
+    }
+    if (dd::launch_transpose(plan->in_dtype, tp, st) != 0) return DD_ERR_CUDA;
+    if (e1) {
+        cudaEventRecord(e1, st);
+        plan->tm_timed = true;
+    }
+    return dd_execute(plan, plan->d_in_own, d_out, cuda_stream);
+}
+
+int dd_plan_transpose_time(dd_plan *plan, float *ms)
+{
+    if (!plan || !ms || !plan->tm_timed) return DD_ERR_INVALID_ARG;
+    if (cudaEventSynchronize(plan->ev_tm[1]) != cudaSuccess ||
+        cudaEventElapsedTime(ms, plan->ev_tm[0], plan->ev_tm[1]) != cudaSuccess)
+        return DD_ERR_CUDA;
+    return DD_OK;
+}
+
 int dd_plan_set_timing(dd_plan *plan, int on)
 {
     if (!plan) return DD_ERR_INVALID_ARG;
@@ -420,7 +465,7 @@ int64_t dd_plan_info(const dd_plan *plan, int what)
     case DD_INFO_THREADS: return t.shape.threads();
     case DD_INFO_WORKSPACE_BYTES: return plan->workspace_bytes;
     case DD_INFO_STAGE_BYTES: return t.stage_bytes_total;
-    case DD_INFO_LAUNCHES: return 2;
+    case DD_INFO_LAUNCHES: return 2;  // dd_execute; dd_execute_tm launches one more
     case DD_INFO_CH: return t.shape.CH;
     case DD_INFO_NSTAGE: return t.nstage;
     default: return -1;

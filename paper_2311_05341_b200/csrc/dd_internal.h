@@ -94,6 +94,13 @@ struct InterleaveParams {
     int nchunk;  // blocks per channel row: ceil((j_end - j_begin) / (4 * 256)), a thread makes 4 superwords
 };
 
+struct TransposeParams {
+    const void *in;   // [nsamps][nchans]
+    void *out;        // [nchans][nsamps]
+    int64_t nsamps;
+    int64_t nchans;
+};
+
 int num_variants();
 const KernelShape &variant_shape(int v);
 // cudaFuncSetAttribute(max dynamic smem) for variant v; returns cudaError_t as int.
@@ -101,5 +108,6 @@ int variant_prepare(int v, int smem_bytes);
 // Launch the main kernel / the interleave pre-pass on `stream`; return cudaError_t as int.
 int launch_dedisperse(int v, const KernelParams &p, int grid, int smem_bytes, void *stream);
 int launch_interleave(int mode, int VW, const InterleaveParams &p, void *stream);
+int launch_transpose(int mode, const TransposeParams &p, void *stream);
 
 }  // namespace dd

@@ -454,6 +454,75 @@ __global__ void __launch_bounds__(256) interleave_kernel(const InterleaveParams 
     for (int i = 0; i < VW; ++i) dst[i] = make_uint4(w[4 * i], w[4 * i + 1], w[4 * i + 2], w[4 * i + 3]);
 }
 
+// ------------------------------------------------------------------ transpose pre-step
+// Time-major filterbank [nsamps][nchans] (how telescopes write it) -> channel-major
+// [nchans][nsamps] (what Eq. 3 / Alg. 3 index); the paper counts this step
+// in its pipeline time.  HBM-bound: every byte is read once and written once.
+// A CTA moves a tile of TC = 32*P channels x TT = 32*P samples (P = elements per 32-bit word).
+// Phase 1: a thread loads P words from P consecutive time rows (coalesced along channels),
+// transposes the P x P elements in registers and stores P words into the transposed
+// shared-memory tile.  Phase 2: rows of that tile (one channel, 32*P samples) go out as
+// coalesced word stores.  Ragged edges and rows that are not 4-byte aligned take an
+// element-wise path through the same tile.
+template <typename T>
+__global__ void __launch_bounds__(256) transpose_kernel(const TransposeParams p)
+{
+    constexpr int P = 4 / static_cast<int>(sizeof(T));
+    constexpr int TC = 32 * P, TT = 32 * P;
+    __shared__ uint32_t tile[TC][33];  // [channel in tile][word along time], +1 word: bank spread
+    const T *in = static_cast<const T *>(p.in);
+    T *out = static_cast<T *>(p.out);
+    const int64_t t0 = static_cast<int64_t>(blockIdx.x) * TT;
+    const int c0 = static_cast<int>(blockIdx.y) * TC;
+    const bool full = t0 + TT <= p.nsamps && c0 + TC <= p.nchans;
+    const bool in_al = (reinterpret_cast<uintptr_t>(in) & 3u) == 0 && (p.nchans * sizeof(T)) % 4 == 0;
+    const bool out_al = (reinterpret_cast<uintptr_t>(out) & 3u) == 0 && (p.nsamps * sizeof(T)) % 4 == 0;
+    if (full && in_al) {
+        for (int q = threadIdx.x; q < 32 * 32; q += 256) {
+            const int cg = q & 31, tg = q >> 5;  // word along channels, group of P time rows
+            uint32_t r[P];
+#pragma unroll
+            for (int i = 0; i < P; ++i)
+                r[i] = *reinterpret_cast<const uint32_t *>(in + (t0 + tg * P + i) * p.nchans + c0 + cg * P);
+            if constexpr (P == 4) {
+                const uint32_t a = __byte_perm(r[0], r[1], 0x5140), b = __byte_perm(r[0], r[1], 0x7362);
+                const uint32_t c = __byte_perm(r[2], r[3], 0x5140), d = __byte_perm(r[2], r[3], 0x7362);
+                tile[cg * 4 + 0][tg] = __byte_perm(a, c, 0x5410);
+                tile[cg * 4 + 1][tg] = __byte_perm(a, c, 0x7632);
+                tile[cg * 4 + 2][tg] = __byte_perm(b, d, 0x5410);
+                tile[cg * 4 + 3][tg] = __byte_perm(b, d, 0x7632);
+            } else if constexpr (P == 2) {
+                tile[cg * 2 + 0][tg] = __byte_perm(r[0], r[1], 0x5410);
+                tile[cg * 2 + 1][tg] = __byte_perm(r[0], r[1], 0x7632);
+            } else {
+                tile[cg][tg] = r[0];
+            }
+        }
+    } else {
+        T *te = reinterpret_cast<T *>(&tile[0][0]);  // element view: row pitch 33 words
+        for (int q = threadIdx.x; q < TC * TT; q += 256) {
+            const int c = q % TC, t = q / TC;
+            T v = 0;
+            if (t0 + t < p.nsamps && c0 + c < p.nchans) v = in[(t0 + t) * p.nchans + c0 + c];
+            te[c * (33 * P) + t] = v;
+        }
+    }
+    __syncthreads();
+    if (full && out_al) {
+        for (int q = threadIdx.x; q < TC * 32; q += 256) {
+            const int w = q & 31, c = q >> 5;
+            *reinterpret_cast<uint32_t *>(out + static_cast<int64_t>(c0 + c) * p.nsamps + t0 + w * P) = tile[c][w];
+        }
+    } else {
+        const T *te = reinterpret_cast<const T *>(&tile[0][0]);
+        for (int q = threadIdx.x; q < TC * TT; q += 256) {
+            const int t = q % TT, c = q / TT;
+            if (t0 + t < p.nsamps && c0 + c < p.nchans)
+                out[static_cast<int64_t>(c0 + c) * p.nsamps + t0 + t] = te[c * (33 * P) + t];
+        }
+    }
+}
+
 // ------------------------------------------------------------------ variant table
 using KernelFn = void (*)(const KernelParams);
 struct Variant {
@@ -525,6 +594,21 @@ static void launch_interleave_vw(int mode, const InterleaveParams &p, unsigned g
         interleave_kernel<DD_U16, VW><<<grid, 256, 0, st>>>(p);
     else
         interleave_kernel<DD_F32, VW><<<grid, 256, 0, st>>>(p);
+}
+
+int launch_transpose(int mode, const TransposeParams &p, void *stream)
+{
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int P = mode == DD_U8 ? 4 : (mode == DD_U16 ? 2 : 1);
+    const dim3 grid(static_cast<unsigned>((p.nsamps + 32 * P - 1) / (32 * P)),
+                    static_cast<unsigned>((p.nchans + 32 * P - 1) / (32 * P)));
+    if (mode == DD_U8)
+        transpose_kernel<uint8_t><<<grid, 256, 0, st>>>(p);
+    else if (mode == DD_U16)
+        transpose_kernel<uint16_t><<<grid, 256, 0, st>>>(p);
+    else
+        transpose_kernel<uint32_t><<<grid, 256, 0, st>>>(p);
+    return static_cast<int>(cudaGetLastError());
 }
 
 int launch_interleave(int mode, int VW, const InterleaveParams &p, void *stream)

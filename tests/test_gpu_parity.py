@@ -299,6 +299,44 @@ def test_host_path_pipelined_chunks_match_oracle(B, oracle, dtype, case, monkeyp
         plan.destroy()
 
 
+TM_CASES = [
+    # nchans, nsamps: whole tiles, ragged both ways, rows not 4-byte aligned, tiny
+    (256, 4096), (130, 5003), (37, 999), (1, 300), (129, 1000), (64, 70001),
+]
+
+
+@pytest.mark.parametrize("dtype", [np.uint8, np.uint16, np.float32])
+@pytest.mark.parametrize("shape", TM_CASES)
+def test_time_major_input_matches_oracle_on_transposed_block(B, oracle, dtype, shape):
+    """dd_execute_tm: the transpose pre-step.  The expected result is the
+    oracle run on numpy's transpose of the same time-major block."""
+    import torch
+    nchans, nsamps = shape
+    rng = np.random.default_rng([nchans, nsamps, 11])
+    x_tm = np.ascontiguousarray(_rand_input(rng, dtype, nchans, nsamps).T)  # [nsamps][nchans]
+    dms = np.arange(9) * 7.0
+    f_high, chan_bw, tsamp = 1500.0, -200.0 / nchans, 64e-6
+    code = {np.uint8: B.DD_U8, np.uint16: B.DD_U16, np.float32: B.DD_F32}[dtype]
+    plan = B.Plan(nchans, nsamps, f_high, chan_bw, tsamp, dms, code)
+    try:
+        odt = torch.float32 if dtype == np.float32 else torch.int32
+        d_out = torch.full((plan.ndm, plan.out_len), -7, dtype=odt, device="cuda")
+        # second run from a device pointer that is only 1-element aligned
+        for shift in (0, 1):
+            flat = torch.empty(x_tm.size + shift, dtype=_torch_in(x_tm[:1]).dtype, device="cuda")
+            view = flat[shift:].view(nsamps, nchans)
+            view.copy_(_torch_in(x_tm))
+            d_out.fill_(-7)
+            plan.execute_tm(view, d_out)
+            torch.cuda.synchronize()
+            got = d_out.cpu().numpy()
+            x_cm = np.ascontiguousarray(x_tm.T)
+            check_against_oracle(oracle, x_cm, got if dtype == np.float32 else got.view(np.uint32),
+                                 plan.shift_table(), plan.out_len)
+    finally:
+        plan.destroy()
+
+
 def test_plan_errors_on_gpu(B):
     with pytest.raises(B.DDError) as e:
         B.Plan(4, 32, 1500.0, -25.0, 1e-3, [0.0, 300.0], B.DD_U8)
