@@ -38,6 +38,8 @@
  * 0.0272824109 s; printed 4-channel shift rows; half-to-even through the whole formula;
  * table invariants; closed form in[c][t] = 100c + t; DM=0 == numpy column sum; constant
  * input; single-impulse response; dispersed pulse re-aligns at its DM; literal brute force.
+ * 4-bit: nibble order on a hand-written byte row; equals the u8 transform of the numpy-unpacked
+ * block; literal brute force.
  */
 #include <math.h>
 #include <stdint.h>
@@ -122,6 +124,35 @@ void oracle_dedisperse_u16(const uint16_t *in, int nchans, int64_t nsamps, const
             const uint16_t *x = in + (size_t)c * nsamps + table[(size_t)d * nchans + c];
             for (int64_t t = 0; t < out_len; t++)
                 o[t] += x[t];
+        }
+    }
+}
+
+/*
+ * ---- packed 4-bit input (the paper's third precision) ------------
+ * Reading R14: two samples per byte, the EARLIER sample in the LOW nibble
+ * (sample t of a channel is nibble t & 1 of byte t >> 1 of that channel's row); rows are
+ * nsamps / 2 bytes, nsamps even.  Same definition, uint32 accumulation.
+ */
+static uint32_t u4_sample(const uint8_t *row, int64_t t)
+{
+    uint8_t b = row[t >> 1];
+    return (t & 1) ? (uint32_t)(b >> 4) : (uint32_t)(b & 15u);
+}
+
+void oracle_dedisperse_u4(const uint8_t *in, int nchans, int64_t nsamps, const int32_t *table,
+                          int ndm, int64_t out_len, uint32_t *out)
+{
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int d = 0; d < ndm; d++) {
+        uint32_t *o = out + (size_t)d * out_len;
+        for (int64_t t = 0; t < out_len; t++)
+            o[t] = 0;
+        for (int c = 0; c < nchans; c++) {
+            const uint8_t *row = in + (size_t)c * (nsamps / 2);
+            int64_t s = table[(size_t)d * nchans + c];
+            for (int64_t t = 0; t < out_len; t++)
+                o[t] += u4_sample(row, t + s);
         }
     }
 }

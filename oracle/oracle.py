@@ -52,7 +52,7 @@ def _load():
             lib.oracle_shift_table.restype = c.c_int
             lib.oracle_shift_table.argtypes = [c.c_int, c.c_double, c.c_double, c.c_double,
                                                c.c_void_p, c.c_int, c.c_void_p, c.c_void_p]
-            for name in ("oracle_dedisperse_u8", "oracle_dedisperse_u16"):
+            for name in ("oracle_dedisperse_u8", "oracle_dedisperse_u16", "oracle_dedisperse_u4"):
                 f = getattr(lib, name)
                 f.restype = None
                 f.argtypes = [c.c_void_p, c.c_int, c.c_int64, c.c_void_p, c.c_int, c.c_int64,
@@ -131,6 +131,21 @@ def dedisperse(x: np.ndarray, table: np.ndarray, out_len: int):
     out = np.empty((ndm, out_len), dtype=np.uint32)
     fn = lib.oracle_dedisperse_u8 if code == U8 else lib.oracle_dedisperse_u16
     fn(_ptr(x), nchans, nsamps, _ptr(table), ndm, out_len, _ptr(out))
+    return out
+
+
+def dedisperse_u4(xp: np.ndarray, table: np.ndarray, out_len: int) -> np.ndarray:
+    """Eq. 3 on packed 4-bit input: ``xp`` is uint8 [nchans, nsamps/2], sample t of a channel in
+    nibble t & 1 (low first) of byte t >> 1 (reading R14).  Returns uint32 [ndm, out_len]."""
+    assert xp.ndim == 2 and xp.flags.c_contiguous and xp.dtype == np.uint8
+    table = np.ascontiguousarray(table, dtype=np.int32)
+    nchans, nbytes = xp.shape
+    nsamps = 2 * nbytes
+    ndm = table.shape[0]
+    assert table.shape == (ndm, nchans)
+    assert out_len >= 0 and (table.size == 0 or int(table.max()) + out_len <= nsamps)
+    out = np.empty((ndm, out_len), dtype=np.uint32)
+    _load().oracle_dedisperse_u4(_ptr(xp), nchans, nsamps, _ptr(table), ndm, out_len, _ptr(out))
     return out
 
 

@@ -284,3 +284,42 @@ def test_f32_double_accumulation(oracle):
     x[1, :] = -1e8
     out, ab = oracle.dedisperse(x, tab, 8)
     assert (out == 62 * 0.25).all() and (ab == 2e8 + 62 * 0.25).all()
+
+
+# ------------------------------------------------------------------ packed 4-bit input (R14)
+def _unpack_u4(xp):
+    """numpy statement of reading R14: low nibble first."""
+    out = np.empty((xp.shape[0], xp.shape[1] * 2), dtype=np.uint8)
+    out[:, 0::2] = xp & 15
+    out[:, 1::2] = xp >> 4
+    return out
+
+
+def test_u4_nibble_order_hand_row(oracle):
+    # one channel, bytes 0x21 0x43 0x65 0x87 -> samples 1,2,3,4,5,6,7,8 (low nibble first)
+    xp = np.array([[0x21, 0x43, 0x65, 0x87]], dtype=np.uint8)
+    tab = np.zeros((1, 1), dtype=np.int32)
+    assert oracle.dedisperse_u4(xp, tab, 8).tolist() == [[1, 2, 3, 4, 5, 6, 7, 8]]
+    # a shift of 3 reads samples 4.. ; two channels with shifts (0, 3): 1+4, 2+5, ...
+    xp2 = np.vstack([xp, xp])
+    tab2 = np.array([[0, 3]], dtype=np.int32)
+    assert oracle.dedisperse_u4(xp2, tab2, 5).tolist() == [[5, 7, 9, 11, 13]]
+
+
+@pytest.mark.parametrize("shape", [(8, 64, 5), (1, 40, 3), (5, 34, 1), (3, 50, 4)])
+def test_u4_equals_u8_transform_of_unpacked_block_and_brute_force(oracle, shape):
+    nchans, nsamps, ndm = shape
+    rng = np.random.default_rng([nchans, nsamps, ndm, 4])
+    xp = rng.integers(0, 256, (nchans, nsamps // 2), dtype=np.uint8)
+    x8 = _unpack_u4(xp)
+    tab = np.sort(rng.integers(0, nsamps // 3, (ndm, nchans)), axis=1).astype(np.int32)
+    out_len = nsamps - int(tab.max())
+    got = oracle.dedisperse_u4(xp, tab, out_len)
+    assert np.array_equal(got, oracle.dedisperse(x8, tab, out_len))
+    assert np.array_equal(got, _literal(x8, tab, out_len))
+
+
+def test_u4_constant_fifteen(oracle):
+    xp = np.full((300, 50), 0xFF, dtype=np.uint8)
+    tab = np.tile(np.arange(300, dtype=np.int32) % 7, (2, 1))
+    assert (oracle.dedisperse_u4(xp, tab, 90) == 15 * 300).all()
