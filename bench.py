@@ -118,7 +118,9 @@ def _host_input(cfg):
     rng = np.random.default_rng(cfg.seed)
     if cfg.in_dtype == W.F32:
         return rng.standard_normal((cfg.nchans, cfg.nsamps), dtype=np.float32)
-    hi = 255 if cfg.in_dtype == W.U8 else 65535
+    hi = {W.U8: 255, W.U16: 65535, W.U4: 15}[cfg.in_dtype]
+    if cfg.in_dtype == W.U4:
+        return rng.integers(0, 256, (cfg.nchans, cfg.nsamps // 2), dtype=np.uint8)
     x = np.empty((cfg.nchans, cfg.nsamps), dtype=cfg.np_dtype)
     step = max(1, (1 << 24) // cfg.nsamps)
     for c0 in range(0, cfg.nchans, step):
@@ -140,11 +142,12 @@ def time_oracle(cfg, steps: int, warmup: int, rows_per_step: int | None = None, 
     sub, out_len, nrows = _oracle_sample(cfg, oracle, rows_per_step)
     if x is None:
         x = _host_input(cfg)
+    run = oracle.dedisperse_u4 if cfg.in_dtype == W.U4 else oracle.dedisperse
     for _ in range(warmup):
-        oracle.dedisperse(x, sub[:max(1, min(nrows, threads))], out_len)
+        run(x, sub[:max(1, min(nrows, threads))], out_len)
     t0 = time.perf_counter()
     for _ in range(steps):
-        oracle.dedisperse(x, sub, out_len)
+        run(x, sub, out_len)
     dt = time.perf_counter() - t0
     adds = float(nrows) * out_len * cfg.nchans * steps
     return {"value": adds / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
@@ -156,7 +159,7 @@ def run_reference(args):
     rank, _, world = _dist_env()
     if rank != 0:
         return 0
-    cfg = W.CONFIGS[args.config]
+    cfg = W.ALL_CONFIGS[args.config]
     base, ms = time_oracle(cfg, args.steps, args.warmup)
     line = {"impl": "reference", "metric": METRIC, "value": base["value"], "unit": UNIT,
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
@@ -172,7 +175,8 @@ def run_reference(args):
 def _dtype_name(cfg):
     return {W.U8: "u8 in, packed u16/u32 integer accumulate, u32 out",
             W.U16: "u16 in, u32 integer accumulate, u32 out",
-            W.F32: "f32"}[cfg.in_dtype]
+            W.F32: "f32",
+            W.U4: "u4 in (widened to u8 lanes by the pre-pass), packed u16/u32 integer accumulate, u32 out"}[cfg.in_dtype]
 
 
 def _config_dict(cfg, plan):
@@ -210,7 +214,7 @@ def run_ours(args):
         dist.barrier()
     B.lib()
 
-    cfg = W.CONFIGS[args.config]
+    cfg = W.ALL_CONFIGS[args.config]
     hbm_gbs, sm_max_mhz, peak_kind = _peaks()
     plan = B.Plan(cfg.nchans, cfg.nsamps, cfg.f_high, cfg.chan_bw, cfg.tsamp, cfg.dm_list, cfg.in_dtype)
     table = plan.shift_table() if cfg.npulses else None
@@ -274,7 +278,7 @@ def run_ours(args):
 
     # ---- time-major input: transpose pre-step + the same path
     tm = None
-    if rank == 0:
+    if rank == 0 and cfg.in_dtype != W.U4:  # no nibble transpose yet
         x_tm = x.t().contiguous()
         plan.set_timing(True)
         tms, tot = [], []
@@ -311,8 +315,9 @@ def run_ours(args):
     int_peak = N_SM * INT_LANES_PER_SM_CLK * clk
     smem_peak_gbs = N_SM * SMEM_BYTES_PER_SM_CLK * clk / 1e9
     in_b = W.ELEM_BYTES[cfg.in_dtype]
-    smem_alg_bytes = adds * in_b                      # one sample read from shared memory per add
-    hbm_alg_bytes = cfg.nchans * cfg.nsamps * in_b + plan.ndm * plan.out_len * 4
+    smem_b = 1 if cfg.in_dtype == W.U4 else in_b        # 4-bit samples travel as bytes on chip
+    smem_alg_bytes = adds * smem_b                      # one sample read from shared memory per add
+    hbm_alg_bytes = int(cfg.nchans * cfg.nsamps * in_b) + plan.ndm * plan.out_len * 4
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "r01b_traffic.json")
     if os.path.exists(tpath):
@@ -328,7 +333,7 @@ def run_ours(args):
                                 % hbm_alg_bytes,
                 "peak_kind": "derived (paper Eq. 8): %d SMs x %d B/clk x %.0f MHz (%s sm_max_mhz)"
                              % (N_SM, SMEM_BYTES_PER_SM_CLK, sm_max_mhz, peak_kind),
-                "algorithmic_bytes_per_add": in_b, "adds_per_launch": adds,
+                "algorithmic_bytes_per_add": smem_b, "adds_per_launch": adds,
                 "kernel_ms": main_s * 1e3, "share_of_step": share}
     roofline_alu = {"bound": "alu", "achieved": kadds / 1e12, "peak": int_peak / 1e12, "unit": "Tadd/s",
                     "frac": kadds / int_peak,
@@ -371,7 +376,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="headline", choices=list(W.CONFIGS))
+    ap.add_argument("--config", default="headline", choices=list(W.ALL_CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     args = ap.parse_args()
     if args.impl == "reference":

@@ -31,7 +31,7 @@ extern "C" {
 typedef struct dd_plan dd_plan;
 
 /* in_dtype of dd_plan_create */
-enum { DD_U8 = 0, DD_U16 = 1, DD_F32 = 2 };
+enum { DD_U8 = 0, DD_U16 = 1, DD_F32 = 2, DD_U4 = 3 };
 
 typedef enum dd_status {
     DD_OK = 0,
@@ -60,10 +60,13 @@ int dd_shift_table_build(int nchans, double f_high_MHz, double chan_bw_MHz, doub
  * Create a plan on the CURRENT CUDA device.  Copies dm_list; builds and owns the host shift
  * table, its device-side tiling metadata and a device workspace (the lane-interleaved copy
  * of one input block).  Launches no kernel on the data path.
- *   in_dtype: DD_U8 / DD_U16 / DD_F32.
+ *   in_dtype: DD_U8 / DD_U16 / DD_F32, or DD_U4 = packed 4-bit samples (the paper's third
+ *   precision): two samples per byte, the earlier one in the low nibble,
+ *   rows of nsamps/2 bytes, nsamps even; output uint32.  DD_U4 rows are widened to 8-bit
+ *   lanes by the pre-pass and then run through the 8-bit kernel.
  * Errors (with *out = NULL): DD_ERR_INVALID_ARG (as dd_shift_table_build, plus out == NULL,
  * nsamps <= 0, unknown dtype); DD_ERR_SHIFT_TOO_LARGE (max shift >= nsamps);
- * DD_ERR_OVERFLOW (u8: 255*nchans >= 2^32; u16: 65535*nchans >= 2^32); DD_ERR_ALLOC;
+ * DD_ERR_OVERFLOW (u8: 255*nchans >= 2^32; u16: 65535*nchans >= 2^32; u4: 15*nchans >= 2^32); DD_ERR_ALLOC;
  * DD_ERR_CUDA; DD_ERR_UNSUPPORTED_DEVICE; DD_ERR_UNSUPPORTED_PLAN.
  * Tuning aid: if the environment variable DD_FORCE_VARIANT=<n> is set, entry n of the
  * compiled kernel table (dd_kernels.cu) is used instead of the automatic choice; the

@@ -13,7 +13,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libdd.so")
 
-DD_U8, DD_U16, DD_F32 = 0, 1, 2
+DD_U8, DD_U16, DD_F32, DD_U4 = 0, 1, 2, 3
 DD_OK = 0
 DD_ERR_INVALID_ARG = -1
 DD_ERR_SHIFT_TOO_LARGE = -2

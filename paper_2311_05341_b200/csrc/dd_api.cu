@@ -40,7 +40,14 @@ struct dd_plan {
 
 namespace {
 
-size_t elem_bytes(int dtype) { return dtype == DD_U8 ? 1 : (dtype == DD_U16 ? 2 : 4); }
+// bytes of n consecutive samples of one channel (n even for the packed 4-bit type)
+size_t sample_bytes(int dtype, int64_t n)
+{
+    if (dtype == DD_U4) return static_cast<size_t>(n / 2);
+    return static_cast<size_t>(n) * (dtype == DD_U8 ? 1 : (dtype == DD_U16 ? 2 : 4));
+}
+// the kernel family a dtype runs through (4-bit rows are widened to 8-bit lanes by the pre-pass)
+int kernel_mode(int dtype) { return dtype == DD_U4 ? DD_U8 : dtype; }
 
 void free_device(dd_plan *p)
 {
@@ -99,9 +106,11 @@ int dd_plan_create(dd_plan **out, int nchans, int64_t nsamps, double f_high_MHz,
     if (!out) return DD_ERR_INVALID_ARG;
     *out = nullptr;
     if (!dm_list || nchans <= 0 || ndm <= 0 || nsamps <= 0) return DD_ERR_INVALID_ARG;
-    if (in_dtype != DD_U8 && in_dtype != DD_U16 && in_dtype != DD_F32) return DD_ERR_INVALID_ARG;
+    if (in_dtype != DD_U8 && in_dtype != DD_U16 && in_dtype != DD_F32 && in_dtype != DD_U4)
+        return DD_ERR_INVALID_ARG;
+    if (in_dtype == DD_U4 && (nsamps & 1)) return DD_ERR_INVALID_ARG;  // rows are whole bytes
     // exact uint32 sums (Heimdall's overflow beyond 8192 channels)
-    const uint64_t top = in_dtype == DD_U8 ? 255u : 65535u;
+    const uint64_t top = in_dtype == DD_U4 ? 15u : (in_dtype == DD_U8 ? 255u : 65535u);
     if (in_dtype != DD_F32 && top * static_cast<uint64_t>(nchans) >= (1ull << 32))
         return DD_ERR_OVERFLOW;
 
@@ -148,7 +157,7 @@ int dd_plan_create(dd_plan **out, int nchans, int64_t nsamps, double f_high_MHz,
         const int forced = force ? std::atoi(force) : -1;
         for (int v = 0; v < dd::num_variants() && !found; ++v) {
             const dd::KernelShape &sh = dd::variant_shape(v);
-            if (sh.mode != in_dtype) continue;
+            if (sh.mode != kernel_mode(in_dtype)) continue;
             if (forced >= 0 ? v != forced : sh.tune != 0) continue;
             found = dd::build_tiling(sh, v, p->table.data(), ndm, nchans, p->out_len, p->max_shift,
                                      smem_limit, &p->til);
@@ -288,7 +297,8 @@ int dd_execute(const dd_plan *plan, const void *d_in, void *d_out, void *cuda_st
 int dd_execute_tm(dd_plan *plan, const void *d_in_tm, void *d_out, void *cuda_stream)
 {
     if (!plan || !d_in_tm || !d_out) return DD_ERR_INVALID_ARG;
-    const size_t in_bytes = static_cast<size_t>(plan->nchans) * plan->nsamps * elem_bytes(plan->in_dtype);
+    if (plan->in_dtype == DD_U4) return DD_ERR_UNSUPPORTED_PLAN;  // nibble transpose: not built yet
+    const size_t in_bytes = static_cast<size_t>(plan->nchans) * sample_bytes(plan->in_dtype, plan->nsamps);
     if (!plan->d_in_own && cudaMalloc(&plan->d_in_own, in_bytes) != cudaSuccess) {
         cudaGetLastError();
         plan->d_in_own = nullptr;
@@ -371,8 +381,8 @@ int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_str
 {
     if (!plan || !h_in || !h_out) return DD_ERR_INVALID_ARG;
     const dd::Tiling &t = plan->til;
-    const size_t eb = elem_bytes(plan->in_dtype);
-    const size_t in_bytes = static_cast<size_t>(plan->nchans) * plan->nsamps * eb;
+    const int dt = plan->in_dtype;
+    const size_t in_bytes = static_cast<size_t>(plan->nchans) * sample_bytes(dt, plan->nsamps);
     const size_t out_bytes = static_cast<size_t>(plan->ndm) * plan->out_len * 4;
     if (!plan->d_in_own && cudaMalloc(&plan->d_in_own, in_bytes) != cudaSuccess) {
         cudaGetLastError();
@@ -416,7 +426,7 @@ int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_str
     unsigned char *din = static_cast<unsigned char *>(plan->d_in_own);
     unsigned char *hout = static_cast<unsigned char *>(h_out);
     unsigned char *dout = static_cast<unsigned char *>(plan->d_out_own);
-    const size_t in_pitch = static_cast<size_t>(plan->nsamps) * eb;
+    const size_t in_pitch = sample_bytes(dt, plan->nsamps);
     const size_t out_pitch = static_cast<size_t>(plan->out_len) * 4;
 
     // the copy stream starts after whatever the caller has queued on `st`
@@ -426,17 +436,18 @@ int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_str
     for (int g = 0; g < G; ++g) {
         const int64_t o0 = g * C, o1 = o0 + C < plan->out_len ? o0 + C : plan->out_len;
         const int64_t need = o1 + plan->max_shift;  // <= nsamps
-        if (need > have) {
-            if (cudaMemcpy2DAsync(din + have * eb, in_pitch, hin + have * eb, in_pitch,
-                                  static_cast<size_t>(need - have) * eb, plan->nchans,
+        const int64_t need_c = dt == DD_U4 ? (need + 1) & ~static_cast<int64_t>(1) : need;  // whole bytes
+        if (need_c > have) {
+            if (cudaMemcpy2DAsync(din + sample_bytes(dt, have), in_pitch, hin + sample_bytes(dt, have),
+                                  in_pitch, sample_bytes(dt, need_c - have), plan->nchans,
                                   cudaMemcpyHostToDevice, plan->st_h2d) != cudaSuccess)
                 return DD_ERR_CUDA;
-            have = need;
+            have = need_c;
         }
         cudaEventRecord(plan->ev_in[g], plan->st_h2d);
         cudaStreamWaitEvent(st, plan->ev_in[g], 0);
         const BlockGeom bg = geom_for(plan, o1 - o0, need - o0);
-        const int rc = launch_block(plan, bg, din + o0 * eb, plan->nsamps, dout + o0 * 4,
+        const int rc = launch_block(plan, bg, din + sample_bytes(dt, o0), plan->nsamps, dout + o0 * 4,
                                     plan->out_len, st, nullptr);
         if (rc != DD_OK) return rc;
         cudaEventRecord(plan->ev_done[g], st);

@@ -380,6 +380,37 @@ __global__ void __launch_bounds__(256) interleave_kernel(const InterleaveParams 
     if (c >= p.nchans) {  // padding channel (nchans rounded up to CH): a zero row
 #pragma unroll
         for (int i = 0; i < 4 * VW; ++i) w[i] = 0u;
+    } else if (MODE == DD_U4) {
+        // packed 4-bit rows (two samples per byte, earlier sample in the low nibble) are widened
+        // to the u8 lane layout here; the main kernel is the u8 one
+        const uint8_t *row = static_cast<const uint8_t *>(p.in) + static_cast<size_t>(c) * (p.in_pitch / 2);
+        const bool aligned = (reinterpret_cast<uintptr_t>(row) & 1u) == 0;
+#pragma unroll
+        for (int v = 0; v < VW; ++v) {
+            uint32_t seg[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int64_t t = (v * 4 + k) * p.L + j;  // multiple of 4: starts on a byte
+                uint32_t h = 0;
+                if (aligned && t + 3 < p.nsamps) {
+                    h = *reinterpret_cast<const uint16_t *>(row + (t >> 1));
+                } else {
+                    if (t < p.nsamps) h = row[t >> 1];
+                    if (t + 2 < p.nsamps) h |= static_cast<uint32_t>(row[(t >> 1) + 1]) << 8;
+                    if (t + 1 >= p.nsamps) h &= 0x000Fu;       // odd valid length: drop the
+                    else if (t + 3 >= p.nsamps) h &= 0x0FFFu;  // nibbles past the end
+                }
+                seg[k] = (h & 0x000Fu) | (h & 0x00F0u) << 4 | (h & 0x0F00u) << 8 | (h & 0xF000u) << 12;
+            }
+            const uint32_t t01l = __byte_perm(seg[0], seg[1], 0x5140);
+            const uint32_t t01h = __byte_perm(seg[0], seg[1], 0x7362);
+            const uint32_t t23l = __byte_perm(seg[2], seg[3], 0x5140);
+            const uint32_t t23h = __byte_perm(seg[2], seg[3], 0x7362);
+            w[0 * VW + v] = __byte_perm(t01l, t23l, 0x5410);
+            w[1 * VW + v] = __byte_perm(t01l, t23l, 0x7632);
+            w[2 * VW + v] = __byte_perm(t01h, t23h, 0x5410);
+            w[3 * VW + v] = __byte_perm(t01h, t23h, 0x7632);
+        }
     } else if (MODE == DD_U8) {
         const uint8_t *row = static_cast<const uint8_t *>(p.in) + static_cast<size_t>(c) * p.in_pitch;
         const bool aligned = (reinterpret_cast<uintptr_t>(row) & 3u) == 0;
@@ -588,7 +619,9 @@ int launch_dedisperse(int v, const KernelParams &p, int grid, int smem_bytes, vo
 template <int VW>
 static void launch_interleave_vw(int mode, const InterleaveParams &p, unsigned grid, cudaStream_t st)
 {
-    if (mode == DD_U8)
+    if (mode == DD_U4)
+        interleave_kernel<DD_U4, VW><<<grid, 256, 0, st>>>(p);
+    else if (mode == DD_U8)
         interleave_kernel<DD_U8, VW><<<grid, 256, 0, st>>>(p);
     else if (mode == DD_U16)
         interleave_kernel<DD_U16, VW><<<grid, 256, 0, st>>>(p);

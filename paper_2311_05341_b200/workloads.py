@@ -15,10 +15,10 @@ from dataclasses import dataclass, field
 
 import numpy as np
 
-U8, U16, F32 = 0, 1, 2
-NP_DTYPE = {U8: np.uint8, U16: np.uint16, F32: np.float32}
-DTYPE_NAME = {U8: "u8", U16: "u16", F32: "f32"}
-ELEM_BYTES = {U8: 1, U16: 2, F32: 4}
+U8, U16, F32, U4 = 0, 1, 2, 3   # U4: packed 4-bit, two samples per byte, earlier one in the low nibble
+NP_DTYPE = {U8: np.uint8, U16: np.uint16, F32: np.float32, U4: np.uint8}
+DTYPE_NAME = {U8: "u8", U16: "u16", F32: "f32", U4: "u4"}
+ELEM_BYTES = {U8: 1, U16: 2, F32: 4, U4: 0.5}
 
 
 @dataclass(frozen=True)
@@ -73,14 +73,32 @@ CONFIGS = {
                       seed=4, mean=32768.0, sd=2048.0, note="configs[4]"),
 }
 
+# Workloads beyond BASELINE.json's five (SURVEY.md 8(f) rows); bench.py accepts both sets.
+EXTRA_CONFIGS = {
+    "headline_u4": Config("headline_u4", 8192, 1 << 18, U4, 1500.0, -300.0 / 8192, 64e-6, 1024, 2.0,
+                          seed=5, mean=7.5, sd=2.0,
+                          note="the headline shape at the paper's 4-bit precision (PAPER.md:295, 424); "
+                               "not in BASELINE.json: SURVEY.md 8(f) rank 2"),
+}
+ALL_CONFIGS = {**CONFIGS, **EXTRA_CONFIGS}
+
 TINY_PULSE_T0 = 1000
 
 
 def _quantise(a: np.ndarray, in_dtype: int) -> np.ndarray:
     if in_dtype == F32:
         return a.astype(np.float32)
+    if in_dtype == U4:
+        return pack_u4(np.clip(np.rint(a), 0, 15).astype(np.uint8))
     hi = 255 if in_dtype == U8 else 65535
     return np.clip(np.rint(a), 0, hi).astype(NP_DTYPE[in_dtype])
+
+
+def pack_u4(x8: np.ndarray) -> np.ndarray:
+    """[nchans, nsamps] values 0..15 -> [nchans, nsamps/2] bytes, sample 2i in the low nibble
+    of byte i, sample 2i+1 in the high nibble (data layout only, no method arithmetic)."""
+    assert x8.shape[1] % 2 == 0
+    return (x8[:, 0::2] | (x8[:, 1::2] << 4)).astype(np.uint8)
 
 
 def _noise_float_numpy(cfg: Config, nchans: int, nsamps: int) -> np.ndarray:
@@ -109,10 +127,10 @@ def noise_torch(cfg: Config, device, nchans: int | None = None, nsamps: int | No
     import torch
     nchans = cfg.nchans if nchans is None else nchans
     nsamps = cfg.nsamps if nsamps is None else nsamps
-    tdt = {U8: torch.uint8, U16: torch.uint16, F32: torch.float32}[cfg.in_dtype]
+    tdt = {U8: torch.uint8, U16: torch.uint16, F32: torch.float32, U4: torch.uint8}[cfg.in_dtype]
     g = torch.Generator(device=device)
     g.manual_seed(cfg.seed)
-    out = torch.empty((nchans, nsamps), dtype=tdt, device=device)
+    out = torch.empty((nchans, nsamps // 2 if cfg.in_dtype == U4 else nsamps), dtype=tdt, device=device)
     step = max(1, (1 << 26) // nsamps)
     for c0 in range(0, nchans, step):
         c1 = min(nchans, c0 + step)
@@ -120,6 +138,9 @@ def noise_torch(cfg: Config, device, nchans: int | None = None, nsamps: int | No
         a.mul_(cfg.sd).add_(cfg.mean)
         if cfg.in_dtype == F32:
             out[c0:c1] = a
+        elif cfg.in_dtype == U4:
+            b = a.round_().clamp_(0, 15).to(torch.uint8)
+            out[c0:c1] = b[:, 0::2] | (b[:, 1::2] << 4)
         else:
             hi = 255 if cfg.in_dtype == U8 else 65535
             a.round_().clamp_(0, hi)

@@ -337,6 +337,58 @@ def test_time_major_input_matches_oracle_on_transposed_block(B, oracle, dtype, s
         plan.destroy()
 
 
+# ------------------------------------------------------------------ packed 4-bit input (DD_U4)
+U4_CASES = CASES + [(520, 3000, 9, 2.0, 1500.0, 300.0, 64e-6)]  # > 256 channels: flush path
+
+
+@pytest.mark.parametrize("case", U4_CASES)
+def test_u4_packed_input_matches_oracle(B, oracle, case, monkeypatch):
+    """Two samples per byte, low nibble first (reading R14): device path, host path (3 chunks,
+    odd chunk lengths) and a byte-misaligned device pointer, bit-exact against oracle.dedisperse_u4."""
+    import torch
+    nchans, nsamps, ndm, step, f_high, band, tsamp = case
+    nsamps -= nsamps & 1
+    rng = np.random.default_rng([nchans, nsamps, ndm, 4])
+    xp = rng.integers(0, 256, (nchans, nsamps // 2), dtype=np.uint8)
+    dms = np.arange(ndm) * step
+    plan = B.Plan(nchans, nsamps, f_high, -band / nchans, tsamp, dms, B.DD_U4)
+    try:
+        ref = oracle.dedisperse_u4(xp, plan.shift_table(), plan.out_len)
+        d_out = torch.full((plan.ndm, plan.out_len), -7, dtype=torch.int32, device="cuda")
+        for shift in (0, 1):
+            flat = torch.empty(xp.size + shift, dtype=torch.uint8, device="cuda")
+            view = flat[shift:].view(nchans, nsamps // 2)
+            view.copy_(torch.from_numpy(xp))
+            d_out.fill_(-7)
+            plan.execute(view, d_out)
+            torch.cuda.synchronize()
+            assert np.array_equal(d_out.cpu().numpy().view(np.uint32), ref)
+        monkeypatch.setenv("DD_HOST_CHUNKS", "3")
+        h_out = torch.full((plan.ndm, plan.out_len), -7, dtype=torch.int32).pin_memory()
+        plan.execute_host(torch.from_numpy(xp).pin_memory(), h_out)
+        assert np.array_equal(h_out.numpy().view(np.uint32), ref)
+    finally:
+        plan.destroy()
+
+
+def test_u4_all_fifteen_and_errors(B):
+    import torch
+    nchans, nsamps = 1031, 2000
+    dms = np.arange(5) * 1.0
+    with B.Plan(nchans, nsamps, 1500.0, -0.1, 64e-6, dms, B.DD_U4) as plan:
+        d_in = torch.full((nchans, nsamps // 2), 0xFF, dtype=torch.uint8, device="cuda")
+        d_out = torch.empty((plan.ndm, plan.out_len), dtype=torch.int32, device="cuda")
+        plan.execute(d_in, d_out)
+        torch.cuda.synchronize()
+        assert (d_out == 15 * nchans).all().item()
+        with pytest.raises(B.DDError) as e:
+            plan.execute_tm(d_in, d_out)
+        assert e.value.status == B.DD_ERR_UNSUPPORTED_PLAN
+    with pytest.raises(B.DDError) as e:
+        B.Plan(8, 1001, 1500.0, -1.0, 64e-6, dms, B.DD_U4)  # odd nsamps: rows are not whole bytes
+    assert e.value.status == B.DD_ERR_INVALID_ARG
+
+
 def test_plan_errors_on_gpu(B):
     with pytest.raises(B.DDError) as e:
         B.Plan(4, 32, 1500.0, -25.0, 1e-3, [0.0, 300.0], B.DD_U8)
