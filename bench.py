@@ -180,7 +180,8 @@ def _dtype_name(cfg):
 
 
 def _config_dict(cfg, plan):
-    d = {"workload": cfg.name, "nchans": cfg.nchans, "nsamps": cfg.nsamps, "ndm": cfg.ndm,
+    d = {"workload": cfg.name + ("" if cfg.nsamps == W.ALL_CONFIGS_NSAMPS.get(cfg.name, cfg.nsamps)
+                                 else " (nsamps overridden)"), "nchans": cfg.nchans, "nsamps": cfg.nsamps, "ndm": cfg.ndm,
          "dm_step": cfg.dm_step, "f_high_MHz": cfg.f_high, "chan_bw_MHz": cfg.chan_bw,
          "tsamp_s": cfg.tsamp, "in_dtype": W.DTYPE_NAME[cfg.in_dtype],
          "l2": "input (%.2f GiB) and output are each larger than the 126 MB L2; no flush needed"
@@ -322,7 +323,7 @@ def run_ours(args):
     tpath = os.path.join(ROOT, "profiles", "r01b_traffic.json")
     if os.path.exists(tpath):
         with open(tpath) as f:
-            traffic = json.load(f).get(cfg.name)
+            traffic = None if args.nsamps else json.load(f).get(cfg.name)
     share = main_s / (main_s + il_s)
     # The dominant kernel reads one sample from shared memory per add: its binding roofline is the
     # shared-memory pipe (ncu: 90-99 % of peak wavefronts), reported in bytes.
@@ -371,6 +372,14 @@ def run_ours(args):
     return 0
 
 
+def _apply_overrides(args):
+    if args.nsamps:
+        import dataclasses
+        base = W.ALL_CONFIGS[args.config]
+        W.ALL_CONFIGS[args.config] = dataclasses.replace(base, nsamps=args.nsamps,
+                                                         name=base.name)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -378,7 +387,11 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="headline", choices=list(W.ALL_CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--nsamps", type=int, default=0,
+                    help="override the config's block length (sanity check: adds/s should not depend "
+                         "on the observation length, PAPER.md:287); the line's config says so")
     args = ap.parse_args()
+    _apply_overrides(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

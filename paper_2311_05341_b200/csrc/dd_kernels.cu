@@ -573,27 +573,31 @@ struct Variant {
 // DD_FORCE_VARIANT environment variable only (A/B measurements, profiles/).
 // u8: LDS.64 superwords, 12 DM warps x 6 superwords, odd-lane adds on the fma pipe (FM = 2):
 // the r01 sweep (profiles/r01_tuning.md) measured 58.0 ms on the headline config against
-// 68.3 ms for the LDS.32 / 16-warp / all-alu shape (entry 5).
+// 68.3 ms for the LDS.32 / 16-warp / all-alu shape (entry 7).
 const Variant kVariants[] = {
     //         mode  VW RD RJ  WD  WJ  CH FM NB OW tune
     DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 2, 1, 4, 0),   // 0
     DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 16, 2, 1, 4, 0),   // 1
     DD_VARIANT(DD_U8, 2, 1, 6, 6, 2, 16, 2, 1, 4, 0),    // 2
-    DD_VARIANT(DD_U8, 2, 1, 6, 3, 4, 16, 2, 1, 4, 0),    // 3
-    DD_VARIANT(DD_U8, 2, 1, 6, 1, 12, 8, 2, 1, 4, 0),    // 4
-    DD_VARIANT(DD_U8, 1, 1, 8, 16, 1, 16, 0, 1, 4, 1),   // 5  r01 first shape (A/B only)
-    DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 1, 1, 4, 1),   // 6  W on fma instead of O (A/B only)
-    DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 0, 1, 4, 1),   // 7  all adds on alu (A/B only)
-    DD_VARIANT(DD_U16, 1, 2, 8, 16, 1, 16, 0, 1, 4, 0),  // 8
-    DD_VARIANT(DD_U16, 1, 1, 8, 16, 1, 16, 0, 1, 4, 0),  // 9
-    DD_VARIANT(DD_U16, 1, 1, 8, 4, 4, 16, 0, 1, 4, 0),   // 10
-    DD_VARIANT(DD_U16, 1, 1, 8, 1, 16, 8, 0, 1, 4, 0),   // 11
-    DD_VARIANT(DD_U16, 2, 2, 4, 16, 1, 16, 0, 1, 4, 1),  // 12 LDS.64 (A/B only)
-    DD_VARIANT(DD_F32, 1, 2, 8, 16, 1, 16, 0, 1, 2, 0),  // 13
-    DD_VARIANT(DD_F32, 1, 1, 8, 16, 1, 16, 0, 1, 2, 0),  // 14
-    DD_VARIANT(DD_F32, 1, 1, 8, 4, 4, 16, 0, 1, 2, 0),   // 15
-    DD_VARIANT(DD_F32, 1, 1, 8, 1, 16, 8, 0, 1, 2, 0),   // 16
-    DD_VARIANT(DD_F32, 1, 2, 8, 16, 1, 16, 0, 1, 4, 1),  // 17 32-bit offsets (A/B only)
+    DD_VARIANT(DD_U8, 2, 1, 6, 6, 2, 8, 2, 1, 4, 0),     // 3
+    DD_VARIANT(DD_U8, 2, 1, 6, 3, 4, 8, 2, 1, 4, 0),     // 4
+    DD_VARIANT(DD_U8, 2, 1, 6, 3, 4, 4, 2, 1, 4, 0),     // 5
+    DD_VARIANT(DD_U8, 2, 1, 6, 1, 12, 4, 2, 1, 4, 0),    // 6  one DM per block: always fits
+    DD_VARIANT(DD_U8, 1, 1, 8, 16, 1, 16, 0, 1, 4, 1),   // 7  r01 first shape (A/B only)
+    DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 1, 1, 4, 1),   // 8  W on fma instead of O (A/B only)
+    DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 0, 1, 4, 1),   // 9  all adds on alu (A/B only)
+    DD_VARIANT(DD_U16, 1, 2, 8, 16, 1, 16, 0, 1, 4, 0),  // 10
+    DD_VARIANT(DD_U16, 1, 1, 8, 16, 1, 16, 0, 1, 4, 0),  // 11
+    DD_VARIANT(DD_U16, 1, 1, 8, 4, 4, 16, 0, 1, 4, 0),   // 12
+    DD_VARIANT(DD_U16, 1, 1, 8, 4, 4, 8, 0, 1, 4, 0),    // 13
+    DD_VARIANT(DD_U16, 1, 1, 8, 1, 16, 4, 0, 1, 4, 0),   // 14 one DM per block: always fits
+    DD_VARIANT(DD_U16, 2, 2, 4, 16, 1, 16, 0, 1, 4, 1),  // 15 LDS.64 (A/B only)
+    DD_VARIANT(DD_F32, 1, 2, 8, 16, 1, 16, 0, 1, 2, 0),  // 16
+    DD_VARIANT(DD_F32, 1, 1, 8, 16, 1, 16, 0, 1, 2, 0),  // 17
+    DD_VARIANT(DD_F32, 1, 1, 8, 4, 4, 16, 0, 1, 2, 0),   // 18
+    DD_VARIANT(DD_F32, 1, 1, 8, 4, 4, 8, 0, 1, 2, 0),    // 19
+    DD_VARIANT(DD_F32, 1, 1, 8, 1, 16, 4, 0, 1, 4, 0),   // 20 one DM per block: always fits
+    DD_VARIANT(DD_F32, 1, 2, 8, 16, 1, 16, 0, 1, 4, 1),  // 21 32-bit offsets (A/B only)
 };
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 

@@ -81,6 +81,7 @@ EXTRA_CONFIGS = {
                                "not in BASELINE.json: SURVEY.md 8(f) rank 2"),
 }
 ALL_CONFIGS = {**CONFIGS, **EXTRA_CONFIGS}
+ALL_CONFIGS_NSAMPS = {k: v.nsamps for k, v in ALL_CONFIGS.items()}
 
 TINY_PULSE_T0 = 1000
 
