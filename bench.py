@@ -136,7 +136,7 @@ def time_oracle(cfg, steps: int, warmup: int, rows_per_step: int | None = None, 
     if rows_per_step is None:
         # bounded sample: about 10-20 s of host work for the cpu_baseline leg (one step), about
         # 5-10 s per step for the reference arm (K steps), at the oracle's ~3 G adds/s per core
-        target_adds = (6e11 if steps == 1 else 3e11) * (0.4 if cfg.in_dtype == W.F32 else 1.0)
+        target_adds = (6e11 if steps == 1 else 3e11) * (0.12 if cfg.in_dtype == W.F32 else 1.0)
         mx_rows = int(np.ceil(target_adds / (float(cfg.nsamps) * cfg.nchans)))
         rows_per_step = int(min(cfg.ndm, max(threads, 4, mx_rows)))
     sub, out_len, nrows = _oracle_sample(cfg, oracle, rows_per_step)

@@ -586,15 +586,15 @@ const Variant kVariants[] = {
     DD_VARIANT(DD_U8, 1, 1, 8, 16, 1, 16, 0, 1, 4, 1),   // 7  r01 first shape (A/B only)
     DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 1, 1, 4, 1),   // 8  W on fma instead of O (A/B only)
     DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 0, 1, 4, 1),   // 9  all adds on alu (A/B only)
-    DD_VARIANT(DD_U16, 1, 2, 8, 16, 1, 16, 0, 1, 4, 0),  // 10
+    DD_VARIANT(DD_U16, 2, 1, 8, 16, 1, 16, 0, 1, 4, 0),  // 10 LDS.64, 16 words per offset fetch
     DD_VARIANT(DD_U16, 1, 1, 8, 16, 1, 16, 0, 1, 4, 0),  // 11
     DD_VARIANT(DD_U16, 1, 1, 8, 4, 4, 16, 0, 1, 4, 0),   // 12
     DD_VARIANT(DD_U16, 1, 1, 8, 4, 4, 8, 0, 1, 4, 0),    // 13
     DD_VARIANT(DD_U16, 1, 1, 8, 1, 16, 4, 0, 1, 4, 0),   // 14 one DM per block: always fits
-    DD_VARIANT(DD_U16, 2, 2, 4, 16, 1, 16, 0, 1, 4, 1),  // 15 LDS.64 (A/B only)
-    DD_VARIANT(DD_F32, 1, 2, 8, 16, 1, 16, 0, 1, 2, 0),  // 16
-    DD_VARIANT(DD_F32, 1, 1, 8, 16, 1, 16, 0, 1, 2, 0),  // 17
-    DD_VARIANT(DD_F32, 1, 1, 8, 4, 4, 16, 0, 1, 2, 0),   // 18
+    DD_VARIANT(DD_U16, 1, 2, 8, 16, 1, 16, 0, 1, 4, 1),  // 15 r01b shape: 2 DMs x 8 words (A/B only)
+    DD_VARIANT(DD_F32, 1, 2, 24, 16, 1, 16, 0, 1, 2, 0), // 16 24 words per offset fetch
+    DD_VARIANT(DD_F32, 1, 2, 8, 16, 1, 16, 0, 1, 2, 0),  // 17
+    DD_VARIANT(DD_F32, 1, 1, 8, 16, 1, 16, 0, 1, 2, 0),  // 18
     DD_VARIANT(DD_F32, 1, 1, 8, 4, 4, 8, 0, 1, 2, 0),    // 19
     DD_VARIANT(DD_F32, 1, 1, 8, 1, 16, 4, 0, 1, 4, 0),   // 20 one DM per block: always fits
     DD_VARIANT(DD_F32, 1, 2, 8, 16, 1, 16, 0, 1, 4, 1),  // 21 32-bit offsets (A/B only)
