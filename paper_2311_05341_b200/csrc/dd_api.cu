@@ -409,18 +409,38 @@ int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_str
     // caller's), at least 8 j tiles per chunk so that the grid still fills the GPU
     const int NL = t.shape.lanes();
     const int64_t tile = static_cast<int64_t>(NL) * t.shape.D_J();
-    int want = 6;  // measured best on the headline config (profiles/r01_tuning.md)
-    if (const char *e = std::getenv("DD_HOST_CHUNKS")) {  // explicit request (tests, tuning)
-        want = std::atoi(e);
-    } else {
-        const int64_t by_tiles = plan->out_len / (8 * tile);
-        if (want > by_tiles) want = static_cast<int>(by_tiles);
-    }
-    if (want > dd_plan::kHostChunks) want = dd_plan::kHostChunks;
-    if (want < 1) want = 1;
     const int64_t unit = static_cast<int64_t>(NL) * 16;
-    const int64_t C = ((plan->out_len + want - 1) / want + unit - 1) / unit * unit;
-    const int G = static_cast<int>((plan->out_len + C - 1) / C);
+    int64_t edge[dd_plan::kHostChunks + 1];  // chunk g = output samples [edge[g], edge[g+1])
+    int G = 0;
+    edge[0] = 0;
+    const char *env = std::getenv("DD_HOST_CHUNKS");  // explicit request (tests, tuning): n equal chunks
+    if (!env && plan->out_len >= 64 * tile) {
+        // Tapered schedule: only the first chunk's host->device copy (chunk + max_shift halo) and
+        // the last chunk's device->host copy are exposed, so those two chunks are small; in
+        // between a chunk may grow as long as its copy hides behind the previous chunk's kernels.
+        static const double frac[dd_plan::kHostChunks] = {0.04, 0.07, 0.12, 0.20, 0.25, 0.20, 0.09, 0.03};
+        double cum = 0.0;
+        for (int g = 0; g < dd_plan::kHostChunks; ++g) {
+            cum += frac[g];
+            int64_t e = g + 1 == dd_plan::kHostChunks
+                            ? plan->out_len
+                            : static_cast<int64_t>(cum * static_cast<double>(plan->out_len)) / unit * unit;
+            if (e > edge[G]) edge[++G] = e;
+        }
+    } else {
+        int want = env ? std::atoi(env) : 6;
+        if (!env) {
+            const int64_t by_tiles = plan->out_len / (8 * tile);
+            if (want > by_tiles) want = static_cast<int>(by_tiles);
+        }
+        if (want > dd_plan::kHostChunks) want = dd_plan::kHostChunks;
+        if (want < 1) want = 1;
+        const int64_t C = ((plan->out_len + want - 1) / want + unit - 1) / unit * unit;
+        while (edge[G] < plan->out_len) {
+            const int64_t e = edge[G] + C < plan->out_len ? edge[G] + C : plan->out_len;
+            edge[++G] = e;
+        }
+    }
 
     const unsigned char *hin = static_cast<const unsigned char *>(h_in);
     unsigned char *din = static_cast<unsigned char *>(plan->d_in_own);
@@ -434,7 +454,7 @@ int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_str
     cudaStreamWaitEvent(plan->st_h2d, plan->ev_done[G], 0);
     int64_t have = 0;  // input samples [0, have) of every channel are on their way to the device
     for (int g = 0; g < G; ++g) {
-        const int64_t o0 = g * C, o1 = o0 + C < plan->out_len ? o0 + C : plan->out_len;
+        const int64_t o0 = edge[g], o1 = edge[g + 1];
         const int64_t need = o1 + plan->max_shift;  // <= nsamps
         const int64_t need_c = dt == DD_U4 ? (need + 1) & ~static_cast<int64_t>(1) : need;  // whole bytes
         if (need_c > have) {

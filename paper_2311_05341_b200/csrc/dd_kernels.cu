@@ -500,7 +500,11 @@ __global__ void __launch_bounds__(256) transpose_kernel(const TransposeParams p)
 {
     constexpr int P = 4 / static_cast<int>(sizeof(T));
     constexpr int TC = 32 * P, TT = 32 * P;
-    __shared__ uint32_t tile[TC][33];  // [channel in tile][word along time], +1 word: bank spread
+    // [channel row][word along time], +1 word of pitch; channel c of the tile lives in row
+    // phys(c) = (c % P) * 32 + c / P so that the 32 lanes of a phase-1 store (consecutive channel
+    // words, same k = c % P) hit 32 different banks
+    __shared__ uint32_t tile[TC][33];
+    auto phys = [](int c) { return (c % P) * 32 + c / P; };
     const T *in = static_cast<const T *>(p.in);
     T *out = static_cast<T *>(p.out);
     const int64_t t0 = static_cast<int64_t>(blockIdx.x) * TT;
@@ -518,13 +522,13 @@ __global__ void __launch_bounds__(256) transpose_kernel(const TransposeParams p)
             if constexpr (P == 4) {
                 const uint32_t a = __byte_perm(r[0], r[1], 0x5140), b = __byte_perm(r[0], r[1], 0x7362);
                 const uint32_t c = __byte_perm(r[2], r[3], 0x5140), d = __byte_perm(r[2], r[3], 0x7362);
-                tile[cg * 4 + 0][tg] = __byte_perm(a, c, 0x5410);
-                tile[cg * 4 + 1][tg] = __byte_perm(a, c, 0x7632);
-                tile[cg * 4 + 2][tg] = __byte_perm(b, d, 0x5410);
-                tile[cg * 4 + 3][tg] = __byte_perm(b, d, 0x7632);
+                tile[0 * 32 + cg][tg] = __byte_perm(a, c, 0x5410);
+                tile[1 * 32 + cg][tg] = __byte_perm(a, c, 0x7632);
+                tile[2 * 32 + cg][tg] = __byte_perm(b, d, 0x5410);
+                tile[3 * 32 + cg][tg] = __byte_perm(b, d, 0x7632);
             } else if constexpr (P == 2) {
-                tile[cg * 2 + 0][tg] = __byte_perm(r[0], r[1], 0x5410);
-                tile[cg * 2 + 1][tg] = __byte_perm(r[0], r[1], 0x7632);
+                tile[0 * 32 + cg][tg] = __byte_perm(r[0], r[1], 0x5410);
+                tile[1 * 32 + cg][tg] = __byte_perm(r[0], r[1], 0x7632);
             } else {
                 tile[cg][tg] = r[0];
             }
@@ -535,21 +539,21 @@ __global__ void __launch_bounds__(256) transpose_kernel(const TransposeParams p)
             const int c = q % TC, t = q / TC;
             T v = 0;
             if (t0 + t < p.nsamps && c0 + c < p.nchans) v = in[(t0 + t) * p.nchans + c0 + c];
-            te[c * (33 * P) + t] = v;
+            te[phys(c) * (33 * P) + t] = v;
         }
     }
     __syncthreads();
     if (full && out_al) {
         for (int q = threadIdx.x; q < TC * 32; q += 256) {
             const int w = q & 31, c = q >> 5;
-            *reinterpret_cast<uint32_t *>(out + static_cast<int64_t>(c0 + c) * p.nsamps + t0 + w * P) = tile[c][w];
+            *reinterpret_cast<uint32_t *>(out + static_cast<int64_t>(c0 + c) * p.nsamps + t0 + w * P) = tile[phys(c)][w];
         }
     } else {
         const T *te = reinterpret_cast<const T *>(&tile[0][0]);
         for (int q = threadIdx.x; q < TC * TT; q += 256) {
             const int t = q % TT, c = q / TT;
             if (t0 + t < p.nsamps && c0 + c < p.nchans)
-                out[static_cast<int64_t>(c0 + c) * p.nsamps + t0 + t] = te[c * (33 * P) + t];
+                out[static_cast<int64_t>(c0 + c) * p.nsamps + t0 + t] = te[phys(c) * (33 * P) + t];
         }
     }
 }
