@@ -157,6 +157,40 @@ void oracle_dedisperse_u4(const uint8_t *in, int nchans, int64_t nsamps, const i
     }
 }
 
+/*
+ * ---- time binning (downsampling), a pipeline step before dedispersion --
+ * Reading R15 (the paper names the step and gives no formula): out[c][t] =
+ * sum_{i<factor} in[c][factor*t + i], t < nsamps / factor (a trailing partial bin is dropped),
+ * raw sums like R6, the integer types widened so the sum is exact: u4 -> u8, u8 -> u16;
+ * float32 stays float32 and is summed in ascending i (double here).
+ * in_dtype: 0 = uint8 -> uint16 out, 2 = float32 -> double out, 3 = packed 4-bit -> uint8 out.
+ */
+void oracle_bin_time(const void *in, int in_dtype, int nchans, int64_t nsamps, int factor,
+                     void *out)
+{
+    int64_t nout = nsamps / factor;
+    for (int c = 0; c < nchans; c++) {
+        for (int64_t t = 0; t < nout; t++) {
+            if (in_dtype == 2) {
+                double acc = 0.0;
+                for (int i = 0; i < factor; i++)
+                    acc += (double)((const float *)in)[(size_t)c * nsamps + factor * t + i];
+                ((double *)out)[(size_t)c * nout + t] = acc;
+            } else if (in_dtype == 0) {
+                uint32_t acc = 0;
+                for (int i = 0; i < factor; i++)
+                    acc += ((const uint8_t *)in)[(size_t)c * nsamps + factor * t + i];
+                ((uint16_t *)out)[(size_t)c * nout + t] = (uint16_t)acc;
+            } else {
+                uint32_t acc = 0;
+                for (int i = 0; i < factor; i++)
+                    acc += u4_sample((const uint8_t *)in + (size_t)c * (nsamps / 2), factor * t + i);
+                ((uint8_t *)out)[(size_t)c * nout + t] = (uint8_t)acc;
+            }
+        }
+    }
+}
+
 /* ---- float32 input: double accumulation, ascending c; also sum |in| (R7) ------------- */
 
 void oracle_dedisperse_f32(const float *in, int nchans, int64_t nsamps, const int32_t *table,

@@ -65,6 +65,8 @@ def _load():
                                                      c.c_void_p, c.c_void_p, c.c_void_p,
                                                      c.c_int64, c.c_void_p, c.c_void_p,
                                                      c.c_void_p]
+            lib.oracle_bin_time.restype = None
+            lib.oracle_bin_time.argtypes = [c.c_void_p, c.c_int, c.c_int, c.c_int64, c.c_int, c.c_void_p]
             lib.oracle_omp_threads.restype = c.c_int
             _lib = lib
     return _lib
@@ -146,6 +148,25 @@ def dedisperse_u4(xp: np.ndarray, table: np.ndarray, out_len: int) -> np.ndarray
     assert out_len >= 0 and (table.size == 0 or int(table.max()) + out_len <= nsamps)
     out = np.empty((ndm, out_len), dtype=np.uint32)
     _load().oracle_dedisperse_u4(_ptr(xp), nchans, nsamps, _ptr(table), ndm, out_len, _ptr(out))
+    return out
+
+
+def bin_time(x: np.ndarray, factor: int, packed_u4: bool = False) -> np.ndarray:
+    """Reading R15: out[c][t] = sum of `factor` consecutive samples (trailing partial bin dropped).
+    uint8 -> uint16, float32 -> float64 (exact reference for the float32 kernel), packed 4-bit
+    (``packed_u4``: x is uint8 [nchans, nsamps/2]) -> uint8."""
+    assert x.ndim == 2 and x.flags.c_contiguous and factor >= 1
+    lib = _load()
+    if packed_u4:
+        assert x.dtype == np.uint8
+        nchans, nsamps, code, odt = x.shape[0], 2 * x.shape[1], 3, np.uint8
+    else:
+        code = _dtype_code(x)
+        assert code in (U8, F32)
+        nchans, nsamps = x.shape
+        odt = np.uint16 if code == U8 else np.float64
+    out = np.empty((nchans, nsamps // factor), dtype=odt)
+    lib.oracle_bin_time(_ptr(x), code, nchans, nsamps, int(factor), _ptr(out))
     return out
 
 

@@ -323,3 +323,29 @@ def test_u4_constant_fifteen(oracle):
     xp = np.full((300, 50), 0xFF, dtype=np.uint8)
     tab = np.tile(np.arange(300, dtype=np.int32) % 7, (2, 1))
     assert (oracle.dedisperse_u4(xp, tab, 90) == 15 * 300).all()
+
+
+# ------------------------------------------------------------------ time binning (R15)
+def test_bin_time_hand_row_and_dropped_tail(oracle):
+    x = np.array([[1, 2, 3, 4, 5, 6, 7], [250, 255, 255, 255, 0, 1, 9]], dtype=np.uint8)
+    assert oracle.bin_time(x, 2).tolist() == [[3, 7, 11], [505, 510, 1]]      # 7th sample dropped
+    assert oracle.bin_time(x, 4).tolist() == [[10], [1015]]
+    xp = np.array([[0x21, 0x43, 0xFF, 0xFF]], dtype=np.uint8)                   # samples 1,2,3,4,15,15,15,15
+    assert oracle.bin_time(xp, 4, packed_u4=True).tolist() == [[10, 60]]
+
+
+@pytest.mark.parametrize("factor", [2, 4, 8, 16])
+def test_bin_time_equals_numpy_reshape_sum(oracle, factor):
+    rng = np.random.default_rng(factor)
+    x8 = rng.integers(0, 256, (5, 1003), dtype=np.uint8)
+    n = 1003 // factor
+    assert np.array_equal(oracle.bin_time(x8, factor),
+                          x8[:, :n * factor].reshape(5, n, factor).astype(np.uint32).sum(axis=2))
+    xf = rng.standard_normal((3, 517)).astype(np.float32)
+    n = 517 // factor
+    assert np.allclose(oracle.bin_time(xf, factor),
+                       xf[:, :n * factor].astype(np.float64).reshape(3, n, factor).sum(axis=2), rtol=0, atol=1e-12)
+    xp = rng.integers(0, 256, (4, 400), dtype=np.uint8)
+    n = 800 // factor
+    assert np.array_equal(oracle.bin_time(xp, factor, packed_u4=True),
+                          _unpack_u4(xp)[:, :n * factor].reshape(4, n, factor).astype(np.uint32).sum(axis=2))
