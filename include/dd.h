@@ -112,6 +112,24 @@ int dd_execute_tm(dd_plan *plan, const void *d_in_tm, void *d_out, void *cuda_st
 int dd_plan_transpose_time(dd_plan *plan, float *ms);
 
 /*
+ * Time binning (downsampling), the pipeline step the paper applies per DM range before
+ * dedispersion and counts in its pipeline time (Table 2's plans):
+ *   out[c][t] = sum_{i < factor} in[c][factor*t + i],   t < nsamps / factor
+ * (the paper gives no formula; reading R15: raw sums, a trailing partial bin is
+ * dropped, integer types are widened so that the sum is exact).
+ *   d_in : DEVICE, dense [nchans][nsamps] of in_dtype.
+ *   d_out: DEVICE, dense [nchans][nsamps / factor]: uint16 for DD_U8, uint8 for DD_U4
+ *          (unpacked: one sample per byte), float32 for DD_F32 (summed in ascending i).
+ *   factor: 2, 4, 8 or 16.
+ * The result is a valid input block for a plan made with tsamp*factor, nsamps/factor and the
+ * output's type (DD_U16 / DD_U8 / DD_F32).  Asynchronous on the stream, no allocation.
+ * Errors: DD_ERR_INVALID_ARG (nulls, sizes, factor, odd nsamps for DD_U4),
+ * DD_ERR_UNSUPPORTED_PLAN (DD_U16 input: no wider integer input type), DD_ERR_CUDA.
+ */
+int dd_bin_time(const void *d_in, void *d_out, int nchans, int64_t nsamps, int factor, int in_dtype,
+                void *cuda_stream);
+
+/*
  * The same transform with HOST buffers: h_in [nchans][nsamps], h_out [ndm][out_len].
  * Pipelined over up to 8 time chunks (default: a tapered 8-chunk schedule with a small first
  * and last chunk; environment variable DD_HOST_CHUNKS=<n> asks for n equal chunks): chunk g's input range [o0, o1 + max_shift) of every channel is copied to a

@@ -336,6 +336,25 @@ int dd_plan_transpose_time(dd_plan *plan, float *ms)
     return DD_OK;
 }
 
+int dd_bin_time(const void *d_in, void *d_out, int nchans, int64_t nsamps, int factor, int in_dtype,
+                void *cuda_stream)
+{
+    if (!d_in || !d_out || nchans <= 0 || nsamps <= 0) return DD_ERR_INVALID_ARG;
+    if (factor != 2 && factor != 4 && factor != 8 && factor != 16) return DD_ERR_INVALID_ARG;
+    if (in_dtype == DD_U16) return DD_ERR_UNSUPPORTED_PLAN;  // no wider integer input type to bin into
+    if (in_dtype != DD_U8 && in_dtype != DD_F32 && in_dtype != DD_U4) return DD_ERR_INVALID_ARG;
+    if (in_dtype == DD_U4 && (nsamps & 1)) return DD_ERR_INVALID_ARG;
+    if (nsamps / factor == 0) return DD_ERR_INVALID_ARG;
+    dd::BinParams bp;
+    bp.in = d_in;
+    bp.out = d_out;
+    bp.nsamps = nsamps;
+    bp.nout = nsamps / factor;
+    bp.nchans = nchans;
+    bp.factor = factor;
+    return dd::launch_bin_time(in_dtype, bp, cuda_stream) == 0 ? DD_OK : DD_ERR_CUDA;
+}
+
 int dd_plan_set_timing(dd_plan *plan, int on)
 {
     if (!plan) return DD_ERR_INVALID_ARG;

@@ -101,6 +101,14 @@ struct TransposeParams {
     int64_t nchans;
 };
 
+struct BinParams {
+    const void *in;   // [nchans][nsamps]
+    void *out;        // [nchans][nout], nout = nsamps / factor
+    int64_t nsamps, nout;
+    int64_t out_begin;  // first output column the generic kernel produces (set by launch_bin_time)
+    int nchans, factor;
+};
+
 int num_variants();
 const KernelShape &variant_shape(int v);
 // cudaFuncSetAttribute(max dynamic smem) for variant v; returns cudaError_t as int.
@@ -109,5 +117,6 @@ int variant_prepare(int v, int smem_bytes);
 int launch_dedisperse(int v, const KernelParams &p, int grid, int smem_bytes, void *stream);
 int launch_interleave(int mode, int VW, const InterleaveParams &p, void *stream);
 int launch_transpose(int mode, const TransposeParams &p, void *stream);
+int launch_bin_time(int mode, const BinParams &p, void *stream);
 
 }  // namespace dd

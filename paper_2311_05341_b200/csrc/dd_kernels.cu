@@ -558,6 +558,139 @@ __global__ void __launch_bounds__(256) transpose_kernel(const TransposeParams p)
     }
 }
 
+// ------------------------------------------------------------------ time binning pre-step
+// out[c][t] = sum_{i < F} in[c][F*t + i]  (PAPER.md:295, 370 name the step; reading R15 in
+// raw sums, integer types widened -- u4 -> u8, u8 -> u16 -- float32 summed in
+// ascending i).  HBM-bound: each input byte is read once.  A thread makes four consecutive
+// outputs from 4*F consecutive inputs (word loads when the rows are 4-byte aligned).
+template <int MODE>
+__device__ __forceinline__ uint32_t bin_sample(const void *row, int64_t t)
+{
+    if (MODE == DD_U4) {
+        const uint32_t b = static_cast<const uint8_t *>(row)[t >> 1];
+        return (t & 1) ? b >> 4 : b & 15u;
+    }
+    return static_cast<const uint8_t *>(row)[t];
+}
+
+// Fast path for integer input whose rows are 16-byte aligned: one thread loads one 16-byte
+// piece (16 u8 / 32 u4 samples = NO = 16/F or 32/F whole bins, F | 16), sums in registers and
+// stores NO outputs with one vector store; four pieces per thread in flight.
+template <int MODE, int F>
+__global__ void __launch_bounds__(256) bin_time_fast_kernel(const BinParams p)
+{
+    constexpr int NS = MODE == DD_U4 ? 32 : 16;  // samples per piece
+    constexpr int NO = NS / F;                   // outputs per piece
+    constexpr int OB = MODE == DD_U4 ? 1 : 2;    // bytes per output
+    const int64_t npiece = p.nout / NO;          // whole pieces per row (the rest: bin_time_kernel)
+    const int64_t nchunk = (npiece + 1023) / 1024;
+    const int c = static_cast<int>(blockIdx.x / nchunk);
+    const size_t row_bytes = MODE == DD_U4 ? static_cast<size_t>(p.nsamps / 2) : static_cast<size_t>(p.nsamps);
+    const uint4 *row = reinterpret_cast<const uint4 *>(static_cast<const uint8_t *>(p.in) + c * row_bytes);
+    uint8_t *orow = static_cast<uint8_t *>(p.out) + static_cast<size_t>(c) * p.nout * OB;
+    const int64_t q0 = static_cast<int64_t>(blockIdx.x % nchunk) * 1024 + threadIdx.x;
+    uint4 v[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+        if (q0 + u * 256 < npiece) v[u] = row[q0 + u * 256];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int64_t q = q0 + u * 256;
+        if (q >= npiece) continue;
+        const uint32_t w[4] = {v[u].x, v[u].y, v[u].z, v[u].w};
+        uint32_t sum[NO];
+#pragma unroll
+        for (int o = 0; o < NO; ++o) sum[o] = 0u;
+#pragma unroll
+        for (int b = 0; b < 16; ++b) {
+            const uint32_t byte = (w[b >> 2] >> (8 * (b & 3))) & 0xffu;
+            if (MODE == DD_U4) {
+                sum[(2 * b) / F] += byte & 15u;
+                sum[(2 * b + 1) / F] += byte >> 4;
+            } else {
+                sum[b / F] += byte;
+            }
+        }
+        uint32_t packed[(NO * OB + 3) / 4];
+#pragma unroll
+        for (int i = 0; i < (NO * OB + 3) / 4; ++i) packed[i] = 0u;
+#pragma unroll
+        for (int o = 0; o < NO; ++o) packed[(o * OB) >> 2] |= sum[o] << (8 * ((o * OB) & 3));
+        uint8_t *dst = orow + q * (NO * OB);
+        if constexpr (NO * OB == 16)
+            *reinterpret_cast<uint4 *>(dst) = make_uint4(packed[0], packed[1], packed[2], packed[3]);
+        else if constexpr (NO * OB == 8)
+            *reinterpret_cast<uint2 *>(dst) = make_uint2(packed[0], packed[1]);
+        else if constexpr (NO * OB == 4)
+            *reinterpret_cast<uint32_t *>(dst) = packed[0];
+        else if constexpr (NO * OB == 2)
+            *reinterpret_cast<uint16_t *>(dst) = static_cast<uint16_t>(packed[0]);
+        else
+            *dst = static_cast<uint8_t>(packed[0]);
+    }
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(256) bin_time_kernel(const BinParams p)
+{
+    const int64_t nchunk = (p.nout - p.out_begin + 1023) / 1024;
+    const int c = static_cast<int>(blockIdx.x / nchunk);
+    const int64_t o0 = p.out_begin + (static_cast<int64_t>(blockIdx.x % nchunk) * blockDim.x + threadIdx.x) * 4;
+    if (o0 >= p.nout) return;
+    const int F = p.factor;
+    const int nvalid = p.nout - o0 < 4 ? static_cast<int>(p.nout - o0) : 4;
+    if (MODE == DD_F32) {
+        const float *row = static_cast<const float *>(p.in) + static_cast<size_t>(c) * p.nsamps;
+        float *orow = static_cast<float *>(p.out) + static_cast<size_t>(c) * p.nout;
+        for (int o = 0; o < nvalid; ++o) {
+            float acc = 0.f;
+            for (int i = 0; i < F; ++i) acc += row[(o0 + o) * F + i];
+            orow[o0 + o] = acc;
+        }
+        return;
+    }
+    // integer inputs: bytes per input sample 1 (u8) or 1/2 (u4)
+    const size_t row_bytes = MODE == DD_U4 ? static_cast<size_t>(p.nsamps / 2) : static_cast<size_t>(p.nsamps);
+    const uint8_t *row = static_cast<const uint8_t *>(p.in) + static_cast<size_t>(c) * row_bytes;
+    uint32_t sum[4] = {0u, 0u, 0u, 0u};
+    const int64_t first = o0 * F;                       // first input sample of this thread
+    const int bytes_per_out = MODE == DD_U4 ? F / 2 : F;  // >= 1 (F >= 2)
+    const bool word_ok = nvalid == 4 && (reinterpret_cast<uintptr_t>(row) & 3u) == 0 &&
+                         (bytes_per_out * 4) % 4 == 0 && ((MODE == DD_U4 ? first / 2 : first) & 3) == 0;
+    if (word_ok) {
+        const uint32_t *w = reinterpret_cast<const uint32_t *>(row + (MODE == DD_U4 ? first / 2 : first));
+        // bytes_per_out * 4 bytes = bytes_per_out words in all; output o owns bytes
+        // [o*bytes_per_out, (o+1)*bytes_per_out)
+        for (int k = 0; k < bytes_per_out; ++k) {
+            const uint32_t x = w[k];
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                const uint32_t byte = (x >> (8 * b)) & 0xffu;
+                const int o = (k * 4 + b) / bytes_per_out;
+                sum[o] += MODE == DD_U4 ? (byte & 15u) + (byte >> 4) : byte;
+            }
+        }
+    } else {
+        for (int o = 0; o < nvalid; ++o)
+            for (int i = 0; i < F; ++i) sum[o] += bin_sample<MODE>(row, first + static_cast<int64_t>(o) * F + i);
+    }
+    if (MODE == DD_U8) {
+        uint16_t *orow = static_cast<uint16_t *>(p.out) + static_cast<size_t>(c) * p.nout;
+        if (nvalid == 4 && (reinterpret_cast<uintptr_t>(orow + o0) & 7u) == 0) {
+            *reinterpret_cast<uint2 *>(orow + o0) = make_uint2(sum[0] | sum[1] << 16, sum[2] | sum[3] << 16);
+        } else {
+            for (int o = 0; o < nvalid; ++o) orow[o0 + o] = static_cast<uint16_t>(sum[o]);
+        }
+    } else {
+        uint8_t *orow = static_cast<uint8_t *>(p.out) + static_cast<size_t>(c) * p.nout;
+        if (nvalid == 4 && (reinterpret_cast<uintptr_t>(orow + o0) & 3u) == 0) {
+            *reinterpret_cast<uint32_t *>(orow + o0) = sum[0] | sum[1] << 8 | sum[2] << 16 | sum[3] << 24;
+        } else {
+            for (int o = 0; o < nvalid; ++o) orow[o0 + o] = static_cast<uint8_t>(sum[o]);
+        }
+    }
+}
+
 // ------------------------------------------------------------------ variant table
 using KernelFn = void (*)(const KernelParams);
 struct Variant {
@@ -635,6 +768,54 @@ static void launch_interleave_vw(int mode, const InterleaveParams &p, unsigned g
         interleave_kernel<DD_U16, VW><<<grid, 256, 0, st>>>(p);
     else
         interleave_kernel<DD_F32, VW><<<grid, 256, 0, st>>>(p);
+}
+
+template <int MODE>
+static void launch_bin_fast(const BinParams &p, unsigned grid, cudaStream_t st)
+{
+    switch (p.factor) {
+    case 2: bin_time_fast_kernel<MODE, 2><<<grid, 256, 0, st>>>(p); break;
+    case 4: bin_time_fast_kernel<MODE, 4><<<grid, 256, 0, st>>>(p); break;
+    case 8: bin_time_fast_kernel<MODE, 8><<<grid, 256, 0, st>>>(p); break;
+    default: bin_time_fast_kernel<MODE, 16><<<grid, 256, 0, st>>>(p); break;
+    }
+}
+
+int launch_bin_time(int mode, const BinParams &p_in, void *stream)
+{
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    BinParams p = p_in;
+    p.out_begin = 0;
+    if (mode != DD_F32) {
+        // whole 16-byte pieces through the fast kernel when every row (input and output) is
+        // suitably aligned; the generic kernel finishes the row tails (or does everything)
+        const int NS = mode == DD_U4 ? 32 : 16, OB = mode == DD_U4 ? 1 : 2;
+        const int NO = NS / p.factor;
+        const size_t row_bytes = mode == DD_U4 ? static_cast<size_t>(p.nsamps / 2) : static_cast<size_t>(p.nsamps);
+        const int ost = NO * OB;  // bytes per vector store
+        const bool aligned = (reinterpret_cast<uintptr_t>(p.in) & 15u) == 0 && row_bytes % 16 == 0 &&
+                             (reinterpret_cast<uintptr_t>(p.out) % ost) == 0 &&
+                             (static_cast<size_t>(p.nout) * OB) % ost == 0;
+        const int64_t npiece = p.nout / NO;
+        if (aligned && npiece > 0) {
+            const unsigned grid = static_cast<unsigned>((npiece + 1023) / 1024 * p.nchans);
+            if (mode == DD_U8)
+                launch_bin_fast<DD_U8>(p, grid, st);
+            else
+                launch_bin_fast<DD_U4>(p, grid, st);
+            p.out_begin = npiece * NO;
+        }
+    }
+    if (p.out_begin < p.nout) {
+        const unsigned grid = static_cast<unsigned>((p.nout - p.out_begin + 1023) / 1024 * p.nchans);
+        if (mode == DD_U8)
+            bin_time_kernel<DD_U8><<<grid, 256, 0, st>>>(p);
+        else if (mode == DD_U4)
+            bin_time_kernel<DD_U4><<<grid, 256, 0, st>>>(p);
+        else
+            bin_time_kernel<DD_F32><<<grid, 256, 0, st>>>(p);
+    }
+    return static_cast<int>(cudaGetLastError());
 }
 
 int launch_transpose(int mode, const TransposeParams &p, void *stream)

@@ -417,6 +417,87 @@ def test_large_shift_plans_fall_back_to_smaller_dm_blocks(B, oracle, dtype, case
     check_against_oracle(oracle, x, out, tab, out_len)
 
 
+# ------------------------------------------------------------------ time binning (dd_bin_time, R15)
+BIN_SHAPES = [(64, 4096), (37, 5003), (5, 1001), (1, 70), (130, 20000)]
+
+
+@pytest.mark.parametrize("factor", [2, 4, 8, 16])
+@pytest.mark.parametrize("shape", BIN_SHAPES)
+def test_bin_time_matches_oracle(B, oracle, shape, factor):
+    import torch
+    nchans, nsamps = shape
+    rng = np.random.default_rng([nchans, nsamps, factor])
+    nout = nsamps // factor
+    # u8 -> u16, bit-exact (also from a 1-byte-misaligned device pointer)
+    x8 = rng.integers(0, 256, (nchans, nsamps), dtype=np.uint8)
+    ref8 = oracle.bin_time(x8, factor)
+    for shift in (0, 1):
+        flat = torch.empty(x8.size + shift, dtype=torch.uint8, device="cuda")
+        view = flat[shift:].view(nchans, nsamps)
+        view.copy_(torch.from_numpy(x8))
+        d_out = torch.full((nchans, nout), -1, dtype=torch.int16, device="cuda")
+        B.bin_time(view, d_out, nchans, nsamps, factor, B.DD_U8)
+        torch.cuda.synchronize()
+        assert np.array_equal(d_out.cpu().numpy().view(np.uint16), ref8)
+    # packed u4 -> u8, bit-exact
+    ns4 = nsamps - (nsamps & 1)
+    xp = rng.integers(0, 256, (nchans, ns4 // 2), dtype=np.uint8)
+    if ns4 // factor:
+        d_out = torch.full((nchans, ns4 // factor), 7, dtype=torch.uint8, device="cuda")
+        B.bin_time(torch.from_numpy(xp).cuda(), d_out, nchans, ns4, factor, B.DD_U4)
+        torch.cuda.synchronize()
+        assert np.array_equal(d_out.cpu().numpy(), oracle.bin_time(xp, factor, packed_u4=True))
+    # f32: float accumulation of <= 16 terms against the double oracle, and bit-exact on integers
+    xf = rng.standard_normal((nchans, nsamps)).astype(np.float32)
+    d_out = torch.empty((nchans, nout), dtype=torch.float32, device="cuda")
+    B.bin_time(torch.from_numpy(xf).cuda(), d_out, nchans, nsamps, factor, B.DD_F32)
+    torch.cuda.synchronize()
+    ab = oracle.bin_time(np.abs(xf), factor)
+    assert (np.abs(d_out.cpu().numpy().astype(np.float64) - oracle.bin_time(xf, factor)) <= 1e-6 * ab + 1e-30).all()
+    xi = rng.integers(0, 1000, (nchans, nsamps)).astype(np.float32)
+    B.bin_time(torch.from_numpy(xi).cuda(), d_out, nchans, nsamps, factor, B.DD_F32)
+    torch.cuda.synchronize()
+    assert np.array_equal(d_out.cpu().numpy().astype(np.float64), oracle.bin_time(xi, factor))
+
+
+def test_binned_range_pipeline_matches_oracle_chain(B, oracle):
+    """One DM range of a Table-2 style plan: bin by 4, then dedisperse the
+    binned block with tsamp*4 -- GPU chain against the oracle chain, bit-exact."""
+    import torch
+    nchans, nsamps, factor = 96, 40000, 4
+    f_high, chan_bw, tsamp = 1500.0, -2.0, 64e-6
+    dms = 100.0 + np.arange(40) * 2.0
+    rng = np.random.default_rng(31)
+    x8 = rng.integers(0, 256, (nchans, nsamps), dtype=np.uint8)
+    nb = nsamps // factor
+    d_bin = torch.empty((nchans, nb), dtype=torch.int16, device="cuda")
+    B.bin_time(torch.from_numpy(x8).cuda(), d_bin, nchans, nsamps, factor, B.DD_U8)
+    with B.Plan(nchans, nb, f_high, chan_bw, tsamp * factor, dms, B.DD_U16) as plan:
+        d_out = torch.empty((plan.ndm, plan.out_len), dtype=torch.int32, device="cuda")
+        plan.execute(d_bin.view(torch.uint16), d_out)
+        torch.cuda.synchronize()
+        otab, omx = oracle.shift_table(nchans, f_high, chan_bw, tsamp * factor, dms)
+        ref = oracle.dedisperse(oracle.bin_time(x8, factor), otab, nb - omx)
+        assert plan.out_len == nb - omx
+        assert np.array_equal(d_out.cpu().numpy().view(np.uint32), ref)
+
+
+def test_bin_time_errors(B):
+    import torch
+    x = torch.zeros((4, 64), dtype=torch.uint8, device="cuda")
+    o = torch.zeros((4, 64), dtype=torch.int16, device="cuda")
+    for factor in (0, 1, 3, 32):
+        with pytest.raises(B.DDError) as e:
+            B.bin_time(x, o, 4, 64, factor, B.DD_U8)
+        assert e.value.status == B.DD_ERR_INVALID_ARG
+    with pytest.raises(B.DDError) as e:
+        B.bin_time(x, o, 4, 32, 2, B.DD_U16)
+    assert e.value.status == B.DD_ERR_UNSUPPORTED_PLAN
+    with pytest.raises(B.DDError) as e:
+        B.bin_time(x, o, 4, 63, 2, B.DD_U4)
+    assert e.value.status == B.DD_ERR_INVALID_ARG
+
+
 def test_plan_errors_on_gpu(B):
     with pytest.raises(B.DDError) as e:
         B.Plan(4, 32, 1500.0, -25.0, 1e-3, [0.0, 300.0], B.DD_U8)
