@@ -41,11 +41,16 @@ class Config:
     pulse_amp: float = 0.0
     pulse_width: int = 0
     npulses: int = 0
+    # multi-range plan (Table 2): ((dm_start, dm_step, count), ...); overrides dm_step
+    dm_ranges: tuple = ()
     note: str = field(default="", compare=False)
 
     @property
     def dm_list(self) -> np.ndarray:
         # one multiply per entry, never a running sum
+        if self.dm_ranges:
+            return np.concatenate([start + np.arange(n, dtype=np.float64) * step
+                                   for start, step, n in self.dm_ranges])
         return np.arange(self.ndm, dtype=np.float64) * self.dm_step
 
     @property
@@ -75,6 +80,14 @@ CONFIGS = {
 
 # Workloads beyond BASELINE.json's five; bench.py accepts both sets.
 EXTRA_CONFIGS = {
+    # The paper's own section 5.2 workload at its largest channel count: 8-bit,
+    # 64 us, 10 s, 1400 MHz centre, 300 MHz band, Table 2's three DM ranges without binning
+    # (3050 trials, DM 0-500).  The paper's figure for it (~5 T adds/s on A100, ~4.5 T on V100,
+    # PAPER.md:424) is an average over 512-8192 channels: context, not a like-for-like baseline.
+    "paper52": Config("paper52", 8192, 156250, U8, 1550.0, -300.0 / 8192, 64e-6, 3050, 0.0,
+                      seed=6, mean=128.0, sd=16.0,
+                      dm_ranges=((0.0, 0.1, 1500), (150.0, 0.2, 750), (300.0, 0.25, 800)),
+                      note="PAPER.md section 5.2 / Table 2 at 8192 channels"),
     "headline_u4": Config("headline_u4", 8192, 1 << 18, U4, 1500.0, -300.0 / 8192, 64e-6, 1024, 2.0,
                           seed=5, mean=7.5, sd=2.0,
                           note="the headline shape at the paper's 4-bit precision (PAPER.md:295, 424); "
