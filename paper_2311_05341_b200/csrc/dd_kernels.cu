@@ -75,7 +75,7 @@ struct Acc;
 
 // FM (u8 only) = which adds are issued as IMAD (x * one + acc, `one` a runtime 1 that ptxas
 // cannot fold) on the fma pipe instead of IADD3 on the alu pipe:
-//   0 none; 1 W += x (both words); 2 O += odd(x) (both words); 3 W += x for the second word only
+//   0 none; 1 W += x (both words); 2 O += odd(x) (both words)
 template <int FM>
 struct Acc<DD_U8, FM> {
     uint32_t W = 0, O = 0;           // packed, flushed every <= 256 channels
@@ -84,9 +84,6 @@ struct Acc<DD_U8, FM> {
     {
         if (FM == 1) {
             W = x * one + W;
-            W = y * one + W;
-        } else if (FM == 3) {
-            W = W + x;
             W = y * one + W;
         } else {
             W = W + x + y;
