@@ -239,3 +239,63 @@ def _stream_ptr(stream) -> int:
     if isinstance(stream, int):
         return stream
     return stream.cuda_stream
+
+
+BIN_OUT_DTYPE = {DD_U8: DD_U16, DD_U4: DD_U8, DD_F32: DD_F32}   # dd_bin_time widens integer types
+
+
+class Survey:
+    """A multi-range DM survey plan in the style of the paper's Table 2: each
+    range is (dm_start, dm_step, count, bin_factor); ranges with bin_factor > 1 run on the
+    time-binned block (dd_bin_time) with tsamp * bin_factor.  Marshalling and a loop only: one
+    dd_plan per range, one binned device buffer per distinct factor, every step in the
+    library's kernels.  ``execute`` returns one output tensor per range."""
+
+    def __init__(self, nchans, nsamps, f_high_MHz, chan_bw_MHz, tsamp_s, ranges, in_dtype):
+        import torch
+        self.nchans, self.nsamps, self.in_dtype = int(nchans), int(nsamps), int(in_dtype)
+        self.ranges, self.plans, self.outs, self.binned = [], [], [], {}
+        tdt = {DD_U8: torch.uint8, DD_U16: torch.uint16, DD_F32: torch.float32}
+        try:
+            for dm_start, dm_step, count, factor in ranges:
+                dms = float(dm_start) + np.arange(int(count), dtype=np.float64) * float(dm_step)
+                factor = int(factor)
+                if factor == 1:
+                    dt, ns, ts = self.in_dtype, self.nsamps, float(tsamp_s)
+                else:
+                    if self.in_dtype not in BIN_OUT_DTYPE:
+                        raise DDError(DD_ERR_UNSUPPORTED_PLAN, "Survey: binning of this input type")
+                    dt, ns, ts = BIN_OUT_DTYPE[self.in_dtype], self.nsamps // factor, float(tsamp_s) * factor
+                    if factor not in self.binned:
+                        self.binned[factor] = torch.empty((self.nchans, ns), dtype=tdt[dt], device="cuda")
+                plan = Plan(nchans, ns, f_high_MHz, chan_bw_MHz, ts, dms, dt)
+                self.plans.append(plan)
+                self.ranges.append((dms, factor))
+                odt = torch.float32 if dt == DD_F32 else torch.int32
+                self.outs.append(torch.empty((plan.ndm, plan.out_len), dtype=odt, device="cuda"))
+        except Exception:
+            self.destroy()
+            raise
+
+    def execute(self, d_in, stream=None):
+        done = set()
+        for plan, (dms, factor), out in zip(self.plans, self.ranges, self.outs):
+            if factor == 1:
+                plan.execute(d_in, out, stream)
+                continue
+            if factor not in done:
+                bin_time(d_in, self.binned[factor], self.nchans, self.nsamps, factor, self.in_dtype, stream)
+                done.add(factor)
+            plan.execute(self.binned[factor], out, stream)
+        return self.outs
+
+    def destroy(self):
+        for p in self.plans:
+            p.destroy()
+        self.plans = []
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()

@@ -168,7 +168,9 @@ int dd_plan_create(dd_plan **out, int nchans, int64_t nsamps, double f_high_MHz,
             return DD_ERR_UNSUPPORTED_PLAN;
         }
         const dd::Tiling &t = p->til;
-        if (dd::variant_prepare(t.variant, static_cast<int>(t.smem_bytes)) != 0) rc = DD_ERR_CUDA;
+        // the attribute is per kernel function, not per plan: always raise it to the device limit
+        // so that plans of one shape with different ring sizes can coexist
+        if (dd::variant_prepare(t.variant, static_cast<int>(smem_limit)) != 0) rc = DD_ERR_CUDA;
         const size_t xbytes = static_cast<size_t>(t.nch_pad) * t.Lw * t.shape.sw_bytes();
         if (rc == DD_OK && cudaMalloc(reinterpret_cast<void **>(&p->d_X), xbytes) != cudaSuccess) {
             cudaGetLastError();

@@ -482,6 +482,65 @@ def test_binned_range_pipeline_matches_oracle_chain(B, oracle):
         assert np.array_equal(d_out.cpu().numpy().view(np.uint32), ref)
 
 
+@pytest.mark.parametrize("dtype", [np.uint8, np.float32])
+def test_multi_range_survey_matches_oracle_chain(B, oracle, dtype):
+    """Three DM ranges with binning 1, 2, 4 (Table-2 style) through
+    binding.Survey against the oracle chain (oracle.bin_time -> oracle.dedisperse) per range."""
+    import torch
+    nchans, nsamps = 80, 30000
+    f_high, chan_bw, tsamp = 1500.0, -2.5, 64e-6
+    ranges = [(0.0, 1.0, 20, 1), (20.0, 2.0, 15, 2), (50.0, 4.0, 10, 4)]
+    rng = np.random.default_rng(17)
+    x = _rand_input(rng, dtype, nchans, nsamps)
+    code = B.DD_U8 if dtype == np.uint8 else B.DD_F32
+    with B.Survey(nchans, nsamps, f_high, chan_bw, tsamp, ranges, code) as sv:
+        outs = sv.execute(_torch_in(x))
+        torch.cuda.synchronize()
+        for (start, step, count, factor), got_t in zip(ranges, outs):
+            dms = start + np.arange(count) * step
+            if factor == 1:
+                xb = x
+            elif dtype == np.uint8:
+                xb = oracle.bin_time(x, factor)                       # uint16
+            else:
+                xb = oracle.bin_time(x, factor).astype(np.float32)    # what the f32 kernel hands on
+            otab, omx = oracle.shift_table(nchans, f_high, chan_bw, tsamp * factor, dms)
+            out_len = xb.shape[1] - omx
+            got = got_t.cpu().numpy()
+            assert got.shape == (count, out_len)
+            if dtype == np.uint8:
+                assert np.array_equal(got.view(np.uint32), oracle.dedisperse(xb, otab, out_len))
+            else:
+                # binned values may differ from the double oracle's rounding by 1 ulp each: compare
+                # against the transform of the GPU's own binned block too (bit-level chain) --
+                # here the tolerance form: 1e-4 * sum |in| as for every f32 plan
+                ref, ab = oracle.dedisperse(xb, otab, out_len)
+                assert (np.abs(got.astype(np.float64) - ref) <= 1e-4 * ab).all()
+
+
+def test_plans_of_one_shape_with_different_ring_sizes_coexist(B, oracle):
+    """The opt-in shared-memory attribute is per kernel function: creating a second plan with a
+    smaller ring must not break launches of an earlier plan with a larger one."""
+    rng = np.random.default_rng(23)
+    big = (96, 30000, np.arange(24) * 6.0)     # long windows -> large stages
+    small = (96, 30000, np.arange(24) * 0.1)   # short windows -> small stages
+    xs, plans = [], []
+    try:
+        for nchans, nsamps, dms in (big, small):
+            xs.append(_rand_input(rng, np.uint8, nchans, nsamps))
+            plans.append(B.Plan(nchans, nsamps, 1500.0, -3.0, 64e-6, dms, B.DD_U8))
+        import torch
+        for x, plan in zip(xs, plans):          # the big plan runs after the small one was created
+            d_out = torch.empty((plan.ndm, plan.out_len), dtype=torch.int32, device="cuda")
+            plan.execute(_torch_in(x), d_out)
+            torch.cuda.synchronize()
+            assert np.array_equal(d_out.cpu().numpy().view(np.uint32),
+                                  oracle.dedisperse(x, plan.shift_table(), plan.out_len))
+    finally:
+        for p in plans:
+            p.destroy()
+
+
 def test_bin_time_errors(B):
     import torch
     x = torch.zeros((4, 64), dtype=torch.uint8, device="cuda")
