@@ -639,6 +639,21 @@ __global__ void __launch_bounds__(256) bin_time_kernel(const BinParams p)
     if (MODE == DD_F32) {
         const float *row = static_cast<const float *>(p.in) + static_cast<size_t>(c) * p.nsamps;
         float *orow = static_cast<float *>(p.out) + static_cast<size_t>(c) * p.nout;
+        if (nvalid == 4 && (reinterpret_cast<uintptr_t>(row + o0 * F) & 15u) == 0 &&
+            (reinterpret_cast<uintptr_t>(orow + o0) & 15u) == 0) {
+            // 4*F consecutive floats as F float4 loads; output o owns floats [o*F, (o+1)*F),
+            // summed in ascending order like the scalar path
+            const float4 *v = reinterpret_cast<const float4 *>(row + o0 * F);
+            float acc[4] = {0.f, 0.f, 0.f, 0.f};
+            for (int k = 0; k < F; ++k) {
+                const float4 x = v[k];
+                const float e[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+                for (int i = 0; i < 4; ++i) acc[(k * 4 + i) / F] += e[i];
+            }
+            *reinterpret_cast<float4 *>(orow + o0) = make_float4(acc[0], acc[1], acc[2], acc[3]);
+            return;
+        }
         for (int o = 0; o < nvalid; ++o) {
             float acc = 0.f;
             for (int i = 0; i < F; ++i) acc += row[(o0 + o) * F + i];
