@@ -101,15 +101,21 @@ int dd_execute(const dd_plan *plan, const void *d_in, void *d_out, void *cuda_st
 /*
  * The transform on TIME-MAJOR input, the order telescopes and SIGPROC filterbank files use:
  *   d_in_tm: DEVICE, dense [nsamps][nchans] of the plan's in_dtype (channel 0 = f_high).
- * A transpose kernel writes the channel-major block Eq. 3 / Alg. 3 index
- * into a plan-owned device buffer (allocated on first use), then dd_execute runs on it; the
- * paper counts this transpose in its pipeline time.  Same stream semantics,
- * output and errors as dd_execute, plus DD_ERR_ALLOC.  With timing on
- * (dd_plan_set_timing), dd_plan_transpose_time returns the duration in milliseconds of
- * the latest timed call's transpose kernel (DD_ERR_INVALID_ARG if there is none).
+ * The pre-pass reads the time-major block directly (a fused transpose + lane interleave: the
+ * paper transposes on the GPU and counts it in its pipeline time), then the same
+ * main kernel runs.  Same stream semantics, output, timing hooks and errors as dd_execute;
+ * DD_ERR_UNSUPPORTED_PLAN for DD_U4 plans (no nibble transpose yet).
  */
-int dd_execute_tm(dd_plan *plan, const void *d_in_tm, void *d_out, void *cuda_stream);
-int dd_plan_transpose_time(dd_plan *plan, float *ms);
+int dd_execute_tm(const dd_plan *plan, const void *d_in_tm, void *d_out, void *cuda_stream);
+
+/*
+ * Stand-alone transpose: time-major d_in_tm [nsamps][nchans] -> channel-major d_out
+ * [nchans][nsamps] (the layout dd_execute, dd_execute_host and dd_bin_time take), both DEVICE,
+ * dtype DD_U8 / DD_U16 / DD_F32.  Asynchronous on the stream, no allocation.
+ * Errors: DD_ERR_INVALID_ARG, DD_ERR_UNSUPPORTED_PLAN (DD_U4), DD_ERR_CUDA.
+ */
+int dd_transpose(const void *d_in_tm, void *d_out, int nchans, int64_t nsamps, int dtype,
+                 void *cuda_stream);
 
 /*
  * Time binning (downsampling), the pipeline step the paper applies per DM range before

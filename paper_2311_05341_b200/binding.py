@@ -28,7 +28,7 @@ INFO = {"D_DM": 0, "D_J": 1, "LANES": 2, "L": 3, "SMEM_BYTES": 4, "GRID": 5, "TH
 
 # every symbol include/dd.h declares (tests check the .so exports all of them)
 SYMBOLS = ("dd_shift_table_build", "dd_plan_create", "dd_plan_shift_table", "dd_execute",
-           "dd_execute_host", "dd_execute_tm", "dd_plan_transpose_time", "dd_bin_time", "dd_plan_info", "dd_plan_set_timing", "dd_plan_kernel_times",
+           "dd_execute_host", "dd_execute_tm", "dd_transpose", "dd_bin_time", "dd_plan_info", "dd_plan_set_timing", "dd_plan_kernel_times",
            "dd_plan_destroy", "dd_strerror", "dd_version")
 
 _lib = None
@@ -66,8 +66,8 @@ def lib() -> ctypes.CDLL:
         L.dd_execute_tm.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p]
         L.dd_bin_time.restype = c.c_int
         L.dd_bin_time.argtypes = [c.c_void_p, c.c_void_p, c.c_int, c.c_int64, c.c_int, c.c_int, c.c_void_p]
-        L.dd_plan_transpose_time.restype = c.c_int
-        L.dd_plan_transpose_time.argtypes = [c.c_void_p, c.POINTER(c.c_float)]
+        L.dd_transpose.restype = c.c_int
+        L.dd_transpose.argtypes = [c.c_void_p, c.c_void_p, c.c_int, c.c_int64, c.c_int, c.c_void_p]
         L.dd_plan_info.restype = c.c_int64
         L.dd_plan_info.argtypes = [c.c_void_p, c.c_int]
         L.dd_plan_set_timing.restype = c.c_int
@@ -107,6 +107,14 @@ def dd_shift_table_build(nchans, f_high_MHz, chan_bw_MHz, tsamp_s, dm_list):
     if rc != DD_OK:
         raise DDError(rc, "dd_shift_table_build")
     return table, int(mx.value)
+
+
+def transpose(d_in_tm, d_out, nchans: int, nsamps: int, dtype: int, stream=None) -> None:
+    """dd_transpose: time-major [nsamps][nchans] -> channel-major [nchans][nsamps] (device tensors)."""
+    rc = lib().dd_transpose(_dev_ptr(d_in_tm), _dev_ptr(d_out), int(nchans), int(nsamps), int(dtype),
+                            _stream_ptr(stream))
+    if rc != DD_OK:
+        raise DDError(rc, "dd_transpose")
 
 
 def bin_time(d_in, d_out, nchans: int, nsamps: int, factor: int, in_dtype: int, stream=None) -> None:
@@ -158,19 +166,12 @@ class Plan:
         if rc != DD_OK:
             raise DDError(rc, "dd_execute")
 
-    # -- dd_execute_tm / dd_plan_transpose_time
+    # -- dd_execute_tm
     def execute_tm(self, d_in_tm, d_out, stream=None) -> None:
         """d_in_tm: time-major [nsamps][nchans] torch CUDA tensor (dense) or raw device address."""
         rc = lib().dd_execute_tm(self._h, _dev_ptr(d_in_tm), _dev_ptr(d_out), _stream_ptr(stream))
         if rc != DD_OK:
             raise DDError(rc, "dd_execute_tm")
-
-    def transpose_time(self) -> float:
-        ms = ctypes.c_float(0.0)
-        rc = lib().dd_plan_transpose_time(self._h, ctypes.byref(ms))
-        if rc != DD_OK:
-            raise DDError(rc, "dd_plan_transpose_time")
-        return float(ms.value)
 
     # -- dd_execute_host
     def execute_host(self, h_in, h_out, stream=None) -> None:

@@ -34,8 +34,6 @@ struct dd_plan {
     cudaEvent_t ev[kRing][3] = {};
     bool ev_made = false;
     mutable int64_t timed_count = 0;
-    cudaEvent_t ev_tm[2] = {};  // around the transpose of the latest timed dd_execute_tm
-    bool tm_timed = false;
 };
 
 namespace {
@@ -64,8 +62,6 @@ void free_device(dd_plan *p)
         if (p->ev_made)
             for (auto &triple : p->ev)
                 for (cudaEvent_t e : triple) cudaEventDestroy(e);
-        for (cudaEvent_t e : p->ev_tm)
-            if (e) cudaEventDestroy(e);
         if (p->host_made) {
             for (cudaEvent_t e : p->ev_in) cudaEventDestroy(e);
             for (cudaEvent_t e : p->ev_done) cudaEventDestroy(e);
@@ -237,7 +233,8 @@ BlockGeom geom_for(const dd_plan *plan, int64_t out_len, int64_t nsamps)
 }
 
 int launch_block(const dd_plan *plan, const BlockGeom &g, const void *d_in, int64_t in_pitch,
-                 void *d_out, int64_t out_pitch, cudaStream_t st, const cudaEvent_t *ev)
+                 void *d_out, int64_t out_pitch, cudaStream_t st, const cudaEvent_t *ev,
+                 bool time_major = false)
 {
     const dd::Tiling &t = plan->til;
     if (ev) cudaEventRecord(ev[0], st);
@@ -253,7 +250,9 @@ int launch_block(const dd_plan *plan, const BlockGeom &g, const void *d_in, int6
     ip.j_begin = 0;
     ip.j_end = g.Lw;
     ip.nchunk = static_cast<int>((g.Lw + 1023) / 1024);
-    if (dd::launch_interleave(plan->in_dtype, t.shape.VW, ip, st) != 0) return DD_ERR_CUDA;
+    if ((time_major ? dd::launch_interleave_tm(plan->in_dtype, t.shape.VW, ip, st)
+                    : dd::launch_interleave(plan->in_dtype, t.shape.VW, ip, st)) != 0)
+        return DD_ERR_CUDA;
     if (ev) cudaEventRecord(ev[1], st);
     dd::KernelParams kp;
     kp.X = plan->d_X;
@@ -296,46 +295,31 @@ int dd_execute(const dd_plan *plan, const void *d_in, void *d_out, void *cuda_st
     return rc;
 }
 
-int dd_execute_tm(dd_plan *plan, const void *d_in_tm, void *d_out, void *cuda_stream)
+int dd_execute_tm(const dd_plan *plan, const void *d_in_tm, void *d_out, void *cuda_stream)
 {
     if (!plan || !d_in_tm || !d_out) return DD_ERR_INVALID_ARG;
     if (plan->in_dtype == DD_U4) return DD_ERR_UNSUPPORTED_PLAN;  // nibble transpose: not built yet
-    const size_t in_bytes = static_cast<size_t>(plan->nchans) * sample_bytes(plan->in_dtype, plan->nsamps);
-    if (!plan->d_in_own && cudaMalloc(&plan->d_in_own, in_bytes) != cudaSuccess) {
-        cudaGetLastError();
-        plan->d_in_own = nullptr;
-        return DD_ERR_ALLOC;
-    }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    dd::TransposeParams tp;
-    tp.in = d_in_tm;
-    tp.out = plan->d_in_own;
-    tp.nsamps = plan->nsamps;
-    tp.nchans = plan->nchans;
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (plan->timing) {
-        if (!plan->ev_tm[0] && (cudaEventCreate(&plan->ev_tm[0]) != cudaSuccess ||
-                                cudaEventCreate(&plan->ev_tm[1]) != cudaSuccess))
-            return DD_ERR_CUDA;
-        e0 = plan->ev_tm[0];
-        e1 = plan->ev_tm[1];
-        cudaEventRecord(e0, st);
-    }
-    if (dd::launch_transpose(plan->in_dtype, tp, st) != 0) return DD_ERR_CUDA;
-    if (e1) {
-        cudaEventRecord(e1, st);
-        plan->tm_timed = true;
-    }
-    return dd_execute(plan, plan->d_in_own, d_out, cuda_stream);
+    const cudaEvent_t *ev = plan->timing ? plan->ev[plan->timed_count % dd_plan::kRing] : nullptr;
+    const BlockGeom g = geom_for(plan, plan->out_len, plan->nsamps);
+    // in_pitch = elements per TIME row of the time-major block
+    const int rc = launch_block(plan, g, d_in_tm, plan->nchans, d_out, plan->out_len, st, ev, true);
+    if (rc == DD_OK && ev) ++plan->timed_count;
+    return rc;
 }
 
-int dd_plan_transpose_time(dd_plan *plan, float *ms)
+int dd_transpose(const void *d_in_tm, void *d_out, int nchans, int64_t nsamps, int dtype,
+                 void *cuda_stream)
 {
-    if (!plan || !ms || !plan->tm_timed) return DD_ERR_INVALID_ARG;
-    if (cudaEventSynchronize(plan->ev_tm[1]) != cudaSuccess ||
-        cudaEventElapsedTime(ms, plan->ev_tm[0], plan->ev_tm[1]) != cudaSuccess)
-        return DD_ERR_CUDA;
-    return DD_OK;
+    if (!d_in_tm || !d_out || nchans <= 0 || nsamps <= 0) return DD_ERR_INVALID_ARG;
+    if (dtype == DD_U4) return DD_ERR_UNSUPPORTED_PLAN;
+    if (dtype != DD_U8 && dtype != DD_U16 && dtype != DD_F32) return DD_ERR_INVALID_ARG;
+    dd::TransposeParams tp;
+    tp.in = d_in_tm;
+    tp.out = d_out;
+    tp.nsamps = nsamps;
+    tp.nchans = nchans;
+    return dd::launch_transpose(dtype, tp, cuda_stream) == 0 ? DD_OK : DD_ERR_CUDA;
 }
 
 int dd_bin_time(const void *d_in, void *d_out, int nchans, int64_t nsamps, int factor, int in_dtype,
@@ -517,7 +501,7 @@ int64_t dd_plan_info(const dd_plan *plan, int what)
     case DD_INFO_THREADS: return t.shape.threads();
     case DD_INFO_WORKSPACE_BYTES: return plan->workspace_bytes;
     case DD_INFO_STAGE_BYTES: return t.stage_bytes_total;
-    case DD_INFO_LAUNCHES: return 2;  // dd_execute; dd_execute_tm launches one more
+    case DD_INFO_LAUNCHES: return 2;
     case DD_INFO_CH: return t.shape.CH;
     case DD_INFO_NSTAGE: return t.nstage;
     default: return -1;

@@ -116,6 +116,7 @@ int variant_prepare(int v, int smem_bytes);
 // Launch the main kernel / the interleave pre-pass on `stream`; return cudaError_t as int.
 int launch_dedisperse(int v, const KernelParams &p, int grid, int smem_bytes, void *stream);
 int launch_interleave(int mode, int VW, const InterleaveParams &p, void *stream);
+int launch_interleave_tm(int mode, int VW, const InterleaveParams &p, void *stream);
 int launch_transpose(int mode, const TransposeParams &p, void *stream);
 int launch_bin_time(int mode, const BinParams &p, void *stream);
 

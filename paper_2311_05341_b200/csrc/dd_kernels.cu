@@ -510,12 +510,22 @@ __global__ void __launch_bounds__(256) transpose_kernel(const TransposeParams p)
     const bool in_al = (reinterpret_cast<uintptr_t>(in) & 3u) == 0 && (p.nchans * sizeof(T)) % 4 == 0;
     const bool out_al = (reinterpret_cast<uintptr_t>(out) & 3u) == 0 && (p.nsamps * sizeof(T)) % 4 == 0;
     if (full && in_al) {
-        for (int q = threadIdx.x; q < 32 * 32; q += 256) {
+        uint32_t rr[4][P];  // all 4*P loads of the thread in flight before any is used
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int q = threadIdx.x + 256 * u;
+            const int cg = q & 31, tg = q >> 5;
+#pragma unroll
+            for (int i = 0; i < P; ++i)
+                rr[u][i] = *reinterpret_cast<const uint32_t *>(in + (t0 + tg * P + i) * p.nchans + c0 + cg * P);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int q = threadIdx.x + 256 * u;
             const int cg = q & 31, tg = q >> 5;  // word along channels, group of P time rows
             uint32_t r[P];
 #pragma unroll
-            for (int i = 0; i < P; ++i)
-                r[i] = *reinterpret_cast<const uint32_t *>(in + (t0 + tg * P + i) * p.nchans + c0 + cg * P);
+            for (int i = 0; i < P; ++i) r[i] = rr[u][i];
             if constexpr (P == 4) {
                 const uint32_t a = __byte_perm(r[0], r[1], 0x5140), b = __byte_perm(r[0], r[1], 0x7362);
                 const uint32_t c = __byte_perm(r[2], r[3], 0x5140), d = __byte_perm(r[2], r[3], 0x7362);
@@ -551,6 +561,101 @@ __global__ void __launch_bounds__(256) transpose_kernel(const TransposeParams p)
             const int t = q % TT, c = q / TT;
             if (t0 + t < p.nsamps && c0 + c < p.nchans)
                 out[static_cast<int64_t>(c0 + c) * p.nsamps + t0 + t] = te[phys(c) * (33 * P) + t];
+        }
+    }
+}
+
+// ------------------------------------------------------------------ fused transpose + interleave
+// Time-major input [nsamps][nchans] straight into the lane-interleaved workspace X (what
+// transpose_kernel + interleave_kernel do in two HBM round trips).  A CTA owns TC = 128 bytes
+// of channels x 32 superword columns.  Phase 1: for each of the LANES x 32 time rows the tile
+// needs (t = l*L + j), one warp copies the row's 128 bytes (word loads, coalesced along
+// channels) into shared memory.  Phase 2: a thread gathers the LANES elements of one
+// (channel, column) superword (byte/half/word loads at a 33-word row pitch: conflict-free
+// across the 32 columns of a warp) and stores it; a warp writes 32 consecutive superwords.
+template <typename T, int VW>
+__global__ void __launch_bounds__(256) interleave_tm_kernel(const InterleaveParams p)
+{
+    constexpr int E = static_cast<int>(sizeof(T));
+    constexpr int LPW = 4 / E, NL = VW * LPW;
+    constexpr int TC = 128 / E;               // channels per tile
+    constexpr int TJ = NL > 8 ? 16 : 32;      // superword columns per tile (static smem <= 48 KB)
+    __shared__ uint32_t tile[NL * TJ][33];
+    const T *in = static_cast<const T *>(p.in);
+    const int64_t ncol_tiles = (p.Lw + TJ - 1) / TJ;
+    const int64_t j0 = static_cast<int64_t>(blockIdx.x % ncol_tiles) * TJ;
+    const int c0 = static_cast<int>(blockIdx.x / ncol_tiles) * TC;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const bool in_al = (reinterpret_cast<uintptr_t>(in) & 3u) == 0 && (p.in_pitch * E) % 4 == 0;
+    // ---- phase 1: rows r = l*TJ + j  <->  time l*L + j0 + j, channels c0 .. c0+TC
+    const bool fast = in_al && c0 + TC <= p.nchans;
+    if (fast) {  // all loads of a warp first (NL*TJ/8 independent 128-byte rows in flight), then the stores
+        constexpr int NR = NL * TJ / 8;
+        uint32_t w[NR];
+#pragma unroll
+        for (int i = 0; i < NR; ++i) {
+            const int r = warp + 8 * i;
+            const int64_t t = static_cast<int64_t>(r / TJ) * p.L + j0 + (r % TJ);
+            w[i] = t < p.nsamps ? reinterpret_cast<const uint32_t *>(in + t * p.in_pitch + c0)[lane] : 0u;
+        }
+#pragma unroll
+        for (int i = 0; i < NR; ++i) tile[warp + 8 * i][lane] = w[i];
+    }
+    for (int r = warp; !fast && r < NL * TJ; r += 8) {
+        const int64_t t = static_cast<int64_t>(r / TJ) * p.L + j0 + (r % TJ);
+        uint32_t w = 0u;
+        if (t < p.nsamps) {
+            const T *src = in + t * p.in_pitch + c0;  // in_pitch = nchans: elements per time row
+            if (false) {
+            } else {
+#pragma unroll
+                for (int k = 0; k < LPW; ++k) {
+                    const int c = c0 + lane * LPW + k;
+                    if (c < p.nchans) w |= static_cast<uint32_t>(src[lane * LPW + k]) << (8 * E * k);
+                }
+            }
+        }
+        tile[r][lane] = w;
+    }
+    __syncthreads();
+    // ---- phase 2: a thread takes one column j and one 32-bit word column cw (LPW channels):
+    // it loads that word from each of the NL lane rows (row pitch 33 words: conflict-free
+    // across the columns of a warp), transposes LPW x LPW elements per superword word in
+    // registers and stores LPW superwords (channels cw*LPW + k), each store coalesced along j
+    for (int q = threadIdx.x; q < 32 * TJ; q += 256) {
+        const int j = q % TJ, cw = q / TJ;
+        if (j0 + j >= p.Lw) continue;
+        uint32_t wl[NL];
+#pragma unroll
+        for (int l = 0; l < NL; ++l) wl[l] = tile[l * TJ + j][cw];
+        uint32_t o[LPW][VW];  // o[k][v]: word v of channel cw*LPW + k
+#pragma unroll
+        for (int v = 0; v < VW; ++v) {
+            if constexpr (LPW == 4) {
+                const uint32_t a = __byte_perm(wl[4 * v], wl[4 * v + 1], 0x5140), b2 = __byte_perm(wl[4 * v], wl[4 * v + 1], 0x7362);
+                const uint32_t c2 = __byte_perm(wl[4 * v + 2], wl[4 * v + 3], 0x5140), d2 = __byte_perm(wl[4 * v + 2], wl[4 * v + 3], 0x7362);
+                o[0][v] = __byte_perm(a, c2, 0x5410);
+                o[1][v] = __byte_perm(a, c2, 0x7632);
+                o[2][v] = __byte_perm(b2, d2, 0x5410);
+                o[3][v] = __byte_perm(b2, d2, 0x7632);
+            } else if constexpr (LPW == 2) {
+                o[0][v] = __byte_perm(wl[2 * v], wl[2 * v + 1], 0x5410);
+                o[1][v] = __byte_perm(wl[2 * v], wl[2 * v + 1], 0x7632);
+            } else {
+                o[0][v] = wl[v];
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < LPW; ++k) {
+            const int c = c0 + cw * LPW + k;
+            if (c >= p.nrows) continue;
+            uint32_t *dst = p.X + (static_cast<size_t>(c) * p.Lw + j0 + j) * VW;
+            if constexpr (VW == 1)
+                dst[0] = o[k][0];
+            else if constexpr (VW == 2)
+                *reinterpret_cast<uint2 *>(dst) = make_uint2(o[k][0], o[k][1]);
+            else
+                *reinterpret_cast<uint4 *>(dst) = make_uint4(o[k][0], o[k][1], o[k][2], o[k][3]);
         }
     }
 }
@@ -842,6 +947,34 @@ int launch_transpose(int mode, const TransposeParams &p, void *stream)
         transpose_kernel<uint16_t><<<grid, 256, 0, st>>>(p);
     else
         transpose_kernel<uint32_t><<<grid, 256, 0, st>>>(p);
+    return static_cast<int>(cudaGetLastError());
+}
+
+template <typename T>
+static void launch_interleave_tm_t(int VW, const InterleaveParams &p, unsigned grid, cudaStream_t st)
+{
+    if (VW == 1)
+        interleave_tm_kernel<T, 1><<<grid, 256, 0, st>>>(p);
+    else if (VW == 2)
+        interleave_tm_kernel<T, 2><<<grid, 256, 0, st>>>(p);
+    else
+        interleave_tm_kernel<T, 4><<<grid, 256, 0, st>>>(p);
+}
+
+// p.in is time-major [nsamps][in_pitch = nchans]; fills all Lw columns of all nrows rows of X
+int launch_interleave_tm(int mode, int VW, const InterleaveParams &p, void *stream)
+{
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int E = mode == DD_U8 ? 1 : (mode == DD_U16 ? 2 : 4);
+    const int TC = 128 / E;
+    const int NL = VW * (4 / E), TJ = NL > 8 ? 16 : 32;
+    const unsigned grid = static_cast<unsigned>((p.Lw + TJ - 1) / TJ * ((p.nrows + TC - 1) / TC));
+    if (mode == DD_U8)
+        launch_interleave_tm_t<uint8_t>(VW, p, grid, st);
+    else if (mode == DD_U16)
+        launch_interleave_tm_t<uint16_t>(VW, p, grid, st);
+    else
+        launch_interleave_tm_t<uint32_t>(VW, p, grid, st);
     return static_cast<int>(cudaGetLastError());
 }
 

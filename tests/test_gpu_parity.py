@@ -307,6 +307,21 @@ TM_CASES = [
 
 @pytest.mark.parametrize("dtype", [np.uint8, np.uint16, np.float32])
 @pytest.mark.parametrize("shape", TM_CASES)
+def test_standalone_transpose_equals_numpy(B, dtype, shape):
+    import torch
+    nchans, nsamps = shape
+    rng = np.random.default_rng([nchans, nsamps, 3])
+    x_tm = np.ascontiguousarray(_rand_input(rng, dtype, nchans, nsamps).T)
+    d_out = torch.empty((nchans, nsamps), dtype=_torch_in(x_tm[:1]).dtype, device="cuda")
+    B.transpose(_torch_in(x_tm), d_out, nchans, nsamps,
+                {np.uint8: B.DD_U8, np.uint16: B.DD_U16, np.float32: B.DD_F32}[dtype])
+    torch.cuda.synchronize()
+    got = d_out.view(torch.int16).cpu().numpy().view(np.uint16) if dtype == np.uint16 else d_out.cpu().numpy()
+    assert np.array_equal(got, x_tm.T)
+
+
+@pytest.mark.parametrize("dtype", [np.uint8, np.uint16, np.float32])
+@pytest.mark.parametrize("shape", TM_CASES)
 def test_time_major_input_matches_oracle_on_transposed_block(B, oracle, dtype, shape):
     """dd_execute_tm: the transpose pre-step.  The expected result is the
     oracle run on numpy's transpose of the same time-major block."""
