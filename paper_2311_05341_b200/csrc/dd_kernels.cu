@@ -411,13 +411,25 @@ __global__ void __launch_bounds__(256) interleave_kernel(const InterleaveParams 
     } else if (MODE == DD_U8) {
         const uint8_t *row = static_cast<const uint8_t *>(p.in) + static_cast<size_t>(c) * p.in_pitch;
         const bool aligned = (reinterpret_cast<uintptr_t>(row) & 3u) == 0;
+        // every lane segment in range: issue all 4*VW loads before any is used
+        const bool fast = aligned && (4 * VW - 1) * p.L + j + 3 < p.nsamps;
+        uint32_t pre[VW][4];
+        if (fast) {
+#pragma unroll
+            for (int v = 0; v < VW; ++v)
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    pre[v][k] = *reinterpret_cast<const uint32_t *>(row + (v * 4 + k) * p.L + j);
+        }
 #pragma unroll
         for (int v = 0; v < VW; ++v) {
             uint32_t seg[4];
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
                 const int64_t t = (v * 4 + k) * p.L + j;
-                if (aligned && t + 3 < p.nsamps) {
+                if (fast) {
+                    seg[k] = pre[v][k];
+                } else if (aligned && t + 3 < p.nsamps) {
                     seg[k] = *reinterpret_cast<const uint32_t *>(row + t);
                 } else {
                     seg[k] = sample_or_zero(row, t, p.nsamps) | sample_or_zero(row, t + 1, p.nsamps) << 8 |
@@ -438,13 +450,24 @@ __global__ void __launch_bounds__(256) interleave_kernel(const InterleaveParams 
     } else if (MODE == DD_U16) {
         const uint16_t *row = static_cast<const uint16_t *>(p.in) + static_cast<size_t>(c) * p.in_pitch;
         const bool aligned = (reinterpret_cast<uintptr_t>(row) & 7u) == 0;
+        const bool fast = aligned && (2 * VW - 1) * p.L + j + 3 < p.nsamps;  // all loads up front
+        uint2 pre[VW][2];
+        if (fast) {
+#pragma unroll
+            for (int v = 0; v < VW; ++v)
+#pragma unroll
+                for (int k = 0; k < 2; ++k)
+                    pre[v][k] = *reinterpret_cast<const uint2 *>(row + (v * 2 + k) * p.L + j);
+        }
 #pragma unroll
         for (int v = 0; v < VW; ++v) {
             uint2 seg[2];
 #pragma unroll
             for (int k = 0; k < 2; ++k) {
                 const int64_t t = (v * 2 + k) * p.L + j;
-                if (aligned && t + 3 < p.nsamps) {
+                if (fast) {
+                    seg[k] = pre[v][k];
+                } else if (aligned && t + 3 < p.nsamps) {
                     seg[k] = *reinterpret_cast<const uint2 *>(row + t);
                 } else {
                     seg[k].x = sample_or_zero(row, t, p.nsamps) | sample_or_zero(row, t + 1, p.nsamps) << 16;
@@ -459,11 +482,19 @@ __global__ void __launch_bounds__(256) interleave_kernel(const InterleaveParams 
     } else {
         const uint32_t *row = static_cast<const uint32_t *>(p.in) + static_cast<size_t>(c) * p.in_pitch;
         const bool aligned = (reinterpret_cast<uintptr_t>(row) & 15u) == 0;
+        const bool fast = aligned && (VW - 1) * p.L + j + 3 < p.nsamps;  // all loads up front
+        uint4 pre[VW];
+        if (fast) {
+#pragma unroll
+            for (int v = 0; v < VW; ++v) pre[v] = *reinterpret_cast<const uint4 *>(row + v * p.L + j);
+        }
 #pragma unroll
         for (int v = 0; v < VW; ++v) {
             const int64_t t = v * p.L + j;
             uint4 seg;
-            if (aligned && t + 3 < p.nsamps) {
+            if (fast) {
+                seg = pre[v];
+            } else if (aligned && t + 3 < p.nsamps) {
                 seg = *reinterpret_cast<const uint4 *>(row + t);
             } else {
                 seg.x = sample_or_zero(row, t, p.nsamps);
