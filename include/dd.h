@@ -149,6 +149,15 @@ int dd_bin_time(const void *d_in, void *d_out, int nchans, int64_t nsamps, int f
 int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream);
 
 /*
+ * dd_execute_host for a TIME-MAJOR host block h_in_tm [nsamps][nchans] (how a telescope back
+ * end or a SIGPROC file delivers it).  Same chunk pipeline; a chunk's new samples are one
+ * contiguous range of the block (a plain copy instead of a strided one) and run through the
+ * fused time-major pre-pass of dd_execute_tm.  Errors as dd_execute_host, plus
+ * DD_ERR_UNSUPPORTED_PLAN for DD_U4 plans.
+ */
+int dd_execute_host_tm(dd_plan *plan, const void *h_in_tm, void *h_out, void *cuda_stream);
+
+/*
  * Facts about the plan, for tests and the benchmark.  `what` is one of DD_INFO_*; unknown
  * keys return -1.
  */

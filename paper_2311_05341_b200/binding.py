@@ -28,7 +28,7 @@ INFO = {"D_DM": 0, "D_J": 1, "LANES": 2, "L": 3, "SMEM_BYTES": 4, "GRID": 5, "TH
 
 # every symbol include/dd.h declares (tests check the .so exports all of them)
 SYMBOLS = ("dd_shift_table_build", "dd_plan_create", "dd_plan_shift_table", "dd_execute",
-           "dd_execute_host", "dd_execute_tm", "dd_transpose", "dd_bin_time", "dd_plan_info", "dd_plan_set_timing", "dd_plan_kernel_times",
+           "dd_execute_host", "dd_execute_host_tm", "dd_execute_tm", "dd_transpose", "dd_bin_time", "dd_plan_info", "dd_plan_set_timing", "dd_plan_kernel_times",
            "dd_plan_destroy", "dd_strerror", "dd_version")
 
 _lib = None
@@ -62,6 +62,8 @@ def lib() -> ctypes.CDLL:
         L.dd_execute.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p]
         L.dd_execute_host.restype = c.c_int
         L.dd_execute_host.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p]
+        L.dd_execute_host_tm.restype = c.c_int
+        L.dd_execute_host_tm.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p]
         L.dd_execute_tm.restype = c.c_int
         L.dd_execute_tm.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p]
         L.dd_bin_time.restype = c.c_int
@@ -179,6 +181,12 @@ class Plan:
         rc = lib().dd_execute_host(self._h, _host_ptr(h_in), _host_ptr(h_out), _stream_ptr(stream))
         if rc != DD_OK:
             raise DDError(rc, "dd_execute_host")
+
+    def execute_host_tm(self, h_in_tm, h_out, stream=None) -> None:
+        """h_in_tm: time-major [nsamps][nchans] host buffer; h_out as execute_host."""
+        rc = lib().dd_execute_host_tm(self._h, _host_ptr(h_in_tm), _host_ptr(h_out), _stream_ptr(stream))
+        if rc != DD_OK:
+            raise DDError(rc, "dd_execute_host_tm")
 
     # -- dd_plan_set_timing / dd_plan_kernel_times
     def set_timing(self, on: bool) -> None:

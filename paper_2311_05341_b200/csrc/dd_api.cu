@@ -382,7 +382,22 @@ int dd_plan_kernel_times(dd_plan *plan, int max_n, float *interleave_ms, float *
 // columns travel device->host on a second copy stream.  PCIe is full duplex, so a step costs
 // about max(H2D, kernels, D2H) plus one chunk of fill and drain instead of their sum.  The
 // kernels see a chunk as a smaller block of the same plan (same shift and tiling tables).
+static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream, bool tm);
+
 int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream)
+{
+    return execute_host_impl(plan, h_in, h_out, cuda_stream, false);
+}
+
+int dd_execute_host_tm(dd_plan *plan, const void *h_in_tm, void *h_out, void *cuda_stream)
+{
+    if (plan && plan->in_dtype == DD_U4) return DD_ERR_UNSUPPORTED_PLAN;
+    return execute_host_impl(plan, h_in_tm, h_out, cuda_stream, true);
+}
+
+// tm: the host block is time-major [nsamps][nchans]; a chunk's new samples are then ONE contiguous
+// range of it (a plain 1-D copy) and the chunk runs through the fused time-major pre-pass.
+static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream, bool tm)
 {
     if (!plan || !h_in || !h_out) return DD_ERR_INVALID_ARG;
     const dd::Tiling &t = plan->til;
@@ -463,17 +478,26 @@ int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_str
         const int64_t need = o1 + plan->max_shift;  // <= nsamps
         const int64_t need_c = dt == DD_U4 ? (need + 1) & ~static_cast<int64_t>(1) : need;  // whole bytes
         if (need_c > have) {
-            if (cudaMemcpy2DAsync(din + sample_bytes(dt, have), in_pitch, hin + sample_bytes(dt, have),
-                                  in_pitch, sample_bytes(dt, need_c - have), plan->nchans,
-                                  cudaMemcpyHostToDevice, plan->st_h2d) != cudaSuccess)
-                return DD_ERR_CUDA;
+            cudaError_t ce;
+            if (tm) {
+                const size_t tb = sample_bytes(dt, plan->nchans);  // bytes of one time row
+                ce = cudaMemcpyAsync(din + have * tb, hin + have * tb, static_cast<size_t>(need_c - have) * tb,
+                                     cudaMemcpyHostToDevice, plan->st_h2d);
+            } else {
+                ce = cudaMemcpy2DAsync(din + sample_bytes(dt, have), in_pitch, hin + sample_bytes(dt, have),
+                                       in_pitch, sample_bytes(dt, need_c - have), plan->nchans,
+                                       cudaMemcpyHostToDevice, plan->st_h2d);
+            }
+            if (ce != cudaSuccess) return DD_ERR_CUDA;
             have = need_c;
         }
         cudaEventRecord(plan->ev_in[g], plan->st_h2d);
         cudaStreamWaitEvent(st, plan->ev_in[g], 0);
         const BlockGeom bg = geom_for(plan, o1 - o0, need - o0);
-        const int rc = launch_block(plan, bg, din + sample_bytes(dt, o0), plan->nsamps, dout + o0 * 4,
-                                    plan->out_len, st, nullptr);
+        const int rc = tm ? launch_block(plan, bg, din + o0 * sample_bytes(dt, plan->nchans), plan->nchans,
+                                         dout + o0 * 4, plan->out_len, st, nullptr, true)
+                          : launch_block(plan, bg, din + sample_bytes(dt, o0), plan->nsamps, dout + o0 * 4,
+                                         plan->out_len, st, nullptr);
         if (rc != DD_OK) return rc;
         cudaEventRecord(plan->ev_done[g], st);
         cudaStreamWaitEvent(plan->st_d2h, plan->ev_done[g], 0);

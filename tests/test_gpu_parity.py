@@ -295,6 +295,14 @@ def test_host_path_pipelined_chunks_match_oracle(B, oracle, dtype, case, monkeyp
             got = h_out.numpy()
             check_against_oracle(oracle, x, got if dtype == np.float32 else got.view(np.uint32),
                                  plan.shift_table(), plan.out_len)
+            # the same block delivered time-major
+            h_tm = xt.t().contiguous()
+            h_tm = h_tm.pin_memory() if pinned else h_tm
+            h_out.fill_(-7)
+            plan.execute_host_tm(h_tm, h_out)
+            got = h_out.numpy()
+            check_against_oracle(oracle, x, got if dtype == np.float32 else got.view(np.uint32),
+                                 plan.shift_table(), plan.out_len)
     finally:
         plan.destroy()
 
