@@ -364,10 +364,13 @@ def run_ours(args):
     smem_alg_bytes = adds * smem_b                      # one sample read from shared memory per add
     hbm_alg_bytes = int(cfg.nchans * cfg.nsamps * in_b) + plan.ndm * plan.out_len * 4
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "r01b_traffic.json")
-    if os.path.exists(tpath):
+    tpath = os.path.join(ROOT, "profiles", "r01b_traffic.csv")  # from the ncu captures (r01b_summary.md)
+    if os.path.exists(tpath) and not args.nsamps:
         with open(tpath) as f:
-            traffic = None if args.nsamps else json.load(f).get(cfg.name)
+            for ln in f.read().splitlines()[1:]:
+                k, v = ln.split(",")
+                if k == cfg.name:
+                    traffic = int(v)
     share = main_s / (main_s + il_s)
     # The dominant kernel reads one sample from shared memory per add: its binding roofline is the
     # shared-memory pipe (ncu: 90-99 % of peak wavefronts), reported in bytes.
