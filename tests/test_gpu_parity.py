@@ -580,6 +580,32 @@ def test_bin_time_errors(B):
     assert e.value.status == B.DD_ERR_INVALID_ARG
 
 
+def test_many_channels_up_to_the_uint32_edge(B):
+    """Maximum sizes of the exact integer paths: u16 with the largest accepted channel count
+    (65537 * 65535 = 2^32 - 65536 - 1 fits uint32 by 65536) on all-max input, and u8 with
+    70000 channels of 255 (274 flushes of the packed lanes)."""
+    import torch
+    dms = np.arange(3) * 0.5
+    nchans, nsamps = 65537, 1024
+    with B.Plan(nchans, nsamps, 1500.0, -300.0 / nchans, 64e-6, dms, B.DD_U16) as plan:
+        d_in = torch.full((nchans, nsamps), -1, dtype=torch.int16, device="cuda")  # 0xFFFF
+        d_out = torch.zeros((plan.ndm, plan.out_len), dtype=torch.int32, device="cuda")
+        plan.execute(d_in.view(torch.uint16), d_out)
+        torch.cuda.synchronize()
+        got = d_out.cpu().numpy().view(np.uint32)
+        assert (got == np.uint32(65537 * 65535)).all()
+    with pytest.raises(B.DDError) as e:
+        B.Plan(65538, nsamps, 1500.0, -300.0 / 65538, 64e-6, dms, B.DD_U16)
+    assert e.value.status == B.DD_ERR_OVERFLOW
+    nchans = 70000
+    with B.Plan(nchans, nsamps, 1500.0, -300.0 / nchans, 64e-6, dms, B.DD_U8) as plan:
+        d_in = torch.full((nchans, nsamps), 255, dtype=torch.uint8, device="cuda")
+        d_out = torch.zeros((plan.ndm, plan.out_len), dtype=torch.int32, device="cuda")
+        plan.execute(d_in, d_out)
+        torch.cuda.synchronize()
+        assert (d_out == 255 * nchans).all().item()
+
+
 def test_plan_errors_on_gpu(B):
     with pytest.raises(B.DDError) as e:
         B.Plan(4, 32, 1500.0, -25.0, 1e-3, [0.0, 300.0], B.DD_U8)
