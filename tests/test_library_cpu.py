@@ -131,3 +131,20 @@ def test_product_path_does_not_import_oracle():
                 src = f.read()
             assert "import paper_2311_05341_b200" not in src and "from paper_2311_05341_b200" not in src
             assert "libdd" not in src and "dd.h" not in src
+
+
+def test_header_is_plain_c(tmp_path):
+    """include/dd.h is the C ABI: it must compile as C99 on its own (no C++ or CUDA types) and
+    declare every symbol the binding loads."""
+    import shutil
+    import subprocess
+    gcc = shutil.which("gcc")
+    if gcc is None:
+        pytest.skip("no gcc")
+    src = tmp_path / "use_dd.c"
+    calls = "\n".join("    (void)&%s;" % name for name in B.SYMBOLS)
+    src.write_text('#include "dd.h"\nint main(void) {\n%s\n    return DD_OK;\n}\n' % calls)
+    inc = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "include")
+    res = subprocess.run([gcc, "-std=c99", "-Wall", "-Wextra", "-Werror", "-pedantic", "-I", inc, "-c",
+                          str(src), "-o", str(tmp_path / "use_dd.o")], capture_output=True, text=True)
+    assert res.returncode == 0, res.stderr
