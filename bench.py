@@ -279,7 +279,7 @@ def run_ours(args):
 
     # ---- time-major input: transpose pre-step + the same path
     tm = None
-    if rank == 0 and cfg.in_dtype != W.U4:  # no nibble transpose yet
+    if rank == 0 and cfg.in_dtype != W.U4:  # (the bench has no time-major 4-bit generator)
         x_tm = x.t().contiguous()
         x_cm = torch.empty_like(x)
         tms, tot = [], []

@@ -103,8 +103,9 @@ int dd_execute(const dd_plan *plan, const void *d_in, void *d_out, void *cuda_st
  *   d_in_tm: DEVICE, dense [nsamps][nchans] of the plan's in_dtype (channel 0 = f_high).
  * The pre-pass reads the time-major block directly (a fused transpose + lane interleave: the
  * paper transposes on the GPU and counts it in its pipeline time), then the same
- * main kernel runs.  Same stream semantics, output, timing hooks and errors as dd_execute;
- * DD_ERR_UNSUPPORTED_PLAN for DD_U4 plans (no nibble transpose yet).
+ * main kernel runs.  Same stream semantics, output, timing hooks and errors as dd_execute.
+ * DD_U4 plans: rows of nchans/2 bytes, the EVEN channel of a byte in the low nibble; nchans must
+ * be even (DD_ERR_UNSUPPORTED_PLAN otherwise).
  */
 int dd_execute_tm(const dd_plan *plan, const void *d_in_tm, void *d_out, void *cuda_stream);
 
@@ -152,8 +153,7 @@ int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_str
  * dd_execute_host for a TIME-MAJOR host block h_in_tm [nsamps][nchans] (how a telescope back
  * end or a SIGPROC file delivers it).  Same chunk pipeline; a chunk's new samples are one
  * contiguous range of the block (a plain copy instead of a strided one) and run through the
- * fused time-major pre-pass of dd_execute_tm.  Errors as dd_execute_host, plus
- * DD_ERR_UNSUPPORTED_PLAN for DD_U4 plans.
+ * fused time-major pre-pass of dd_execute_tm.  Errors as dd_execute_host and dd_execute_tm.
  */
 int dd_execute_host_tm(dd_plan *plan, const void *h_in_tm, void *h_out, void *cuda_stream);
 

@@ -298,7 +298,7 @@ int dd_execute(const dd_plan *plan, const void *d_in, void *d_out, void *cuda_st
 int dd_execute_tm(const dd_plan *plan, const void *d_in_tm, void *d_out, void *cuda_stream)
 {
     if (!plan || !d_in_tm || !d_out) return DD_ERR_INVALID_ARG;
-    if (plan->in_dtype == DD_U4) return DD_ERR_UNSUPPORTED_PLAN;  // nibble transpose: not built yet
+    if (plan->in_dtype == DD_U4 && (plan->nchans & 1)) return DD_ERR_UNSUPPORTED_PLAN;  // whole bytes per time row
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const cudaEvent_t *ev = plan->timing ? plan->ev[plan->timed_count % dd_plan::kRing] : nullptr;
     const BlockGeom g = geom_for(plan, plan->out_len, plan->nsamps);
@@ -391,7 +391,7 @@ int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_str
 
 int dd_execute_host_tm(dd_plan *plan, const void *h_in_tm, void *h_out, void *cuda_stream)
 {
-    if (plan && plan->in_dtype == DD_U4) return DD_ERR_UNSUPPORTED_PLAN;
+    if (plan && plan->in_dtype == DD_U4 && (plan->nchans & 1)) return DD_ERR_UNSUPPORTED_PLAN;
     return execute_host_impl(plan, h_in_tm, h_out, cuda_stream, true);
 }
 

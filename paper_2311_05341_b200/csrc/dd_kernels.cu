@@ -691,6 +691,89 @@ __global__ void __launch_bounds__(256) interleave_tm_kernel(const InterleavePara
     }
 }
 
+// The same for packed 4-bit time-major input [nsamps][nchans/2 bytes] (reading R16: the even
+// channel of a byte in the low nibble): a tile is 128 bytes = 256 channels; phase 2 splits each
+// word into its low-nibble and high-nibble bytes (even / odd channels) before the 4 x 4 byte
+// transposes, so a thread stores the u8-lane superwords of eight channels.
+template <int VW>
+__global__ void __launch_bounds__(256) interleave_tm_u4_kernel(const InterleaveParams p)
+{
+    constexpr int NL = VW * 4;
+    constexpr int TJ = NL > 8 ? 16 : 32;
+    __shared__ uint32_t tile[NL * TJ][33];
+    const uint8_t *in = static_cast<const uint8_t *>(p.in);
+    const int64_t pb = p.in_pitch / 2;  // bytes per time row
+    const int64_t ncol_tiles = (p.Lw + TJ - 1) / TJ;
+    const int64_t j0 = static_cast<int64_t>(blockIdx.x % ncol_tiles) * TJ;
+    const int c0 = static_cast<int>(blockIdx.x / ncol_tiles) * 256;  // first channel of the tile
+    const int b0 = c0 / 2;                                           // its byte in a time row
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const bool fast = (reinterpret_cast<uintptr_t>(in) & 3u) == 0 && pb % 4 == 0 && b0 + 128 <= pb;
+    constexpr int NR = NL * TJ / 8;
+    if (fast) {
+        uint32_t w[NR];
+#pragma unroll
+        for (int i = 0; i < NR; ++i) {
+            const int r = warp + 8 * i;
+            const int64_t t = static_cast<int64_t>(r / TJ) * p.L + j0 + (r % TJ);
+            w[i] = t < p.nsamps ? reinterpret_cast<const uint32_t *>(in + t * pb + b0)[lane] : 0u;
+        }
+#pragma unroll
+        for (int i = 0; i < NR; ++i) tile[warp + 8 * i][lane] = w[i];
+    } else {
+        for (int r = warp; r < NL * TJ; r += 8) {
+            const int64_t t = static_cast<int64_t>(r / TJ) * p.L + j0 + (r % TJ);
+            uint32_t w = 0u;
+            if (t < p.nsamps) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const int64_t b = b0 + lane * 4 + k;
+                    if (b < pb) w |= static_cast<uint32_t>(in[t * pb + b]) << (8 * k);
+                }
+            }
+            tile[r][lane] = w;
+        }
+    }
+    __syncthreads();
+    for (int q = threadIdx.x; q < 32 * TJ; q += 256) {
+        const int j = q % TJ, cw = q / TJ;
+        if (j0 + j >= p.Lw) continue;
+        uint32_t o[8][VW];  // o[2*b + parity][v]: word v of channel c0 + cw*8 + 2*b + parity
+#pragma unroll
+        for (int v = 0; v < VW; ++v) {
+            uint32_t lo[4], hi[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const uint32_t w = tile[(4 * v + i) * TJ + j][cw];
+                lo[i] = w & 0x0F0F0F0Fu;
+                hi[i] = (w >> 4) & 0x0F0F0F0Fu;
+            }
+#pragma unroll
+            for (int par = 0; par < 2; ++par) {
+                const uint32_t *x = par ? hi : lo;
+                const uint32_t a = __byte_perm(x[0], x[1], 0x5140), b2 = __byte_perm(x[0], x[1], 0x7362);
+                const uint32_t c2 = __byte_perm(x[2], x[3], 0x5140), d2 = __byte_perm(x[2], x[3], 0x7362);
+                o[0 + par][v] = __byte_perm(a, c2, 0x5410);
+                o[2 + par][v] = __byte_perm(a, c2, 0x7632);
+                o[4 + par][v] = __byte_perm(b2, d2, 0x5410);
+                o[6 + par][v] = __byte_perm(b2, d2, 0x7632);
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const int c = c0 + cw * 8 + k;
+            if (c >= p.nrows) continue;
+            uint32_t *dst = p.X + (static_cast<size_t>(c) * p.Lw + j0 + j) * VW;
+            if constexpr (VW == 1)
+                dst[0] = o[k][0];
+            else if constexpr (VW == 2)
+                *reinterpret_cast<uint2 *>(dst) = make_uint2(o[k][0], o[k][1]);
+            else
+                *reinterpret_cast<uint4 *>(dst) = make_uint4(o[k][0], o[k][1], o[k][2], o[k][3]);
+        }
+    }
+}
+
 // ------------------------------------------------------------------ time binning pre-step
 // out[c][t] = sum_{i < F} in[c][F*t + i]  (PAPER.md:295, 370 name the step; reading R15 in
 // raw sums, integer types widened -- u4 -> u8, u8 -> u16 -- float32 summed in
@@ -996,6 +1079,17 @@ static void launch_interleave_tm_t(int VW, const InterleaveParams &p, unsigned g
 int launch_interleave_tm(int mode, int VW, const InterleaveParams &p, void *stream)
 {
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (mode == DD_U4) {
+        const int TJ4 = VW * 4 > 8 ? 16 : 32;
+        const unsigned g4 = static_cast<unsigned>((p.Lw + TJ4 - 1) / TJ4 * ((p.nrows + 255) / 256));
+        if (VW == 1)
+            interleave_tm_u4_kernel<1><<<g4, 256, 0, st>>>(p);
+        else if (VW == 2)
+            interleave_tm_u4_kernel<2><<<g4, 256, 0, st>>>(p);
+        else
+            interleave_tm_u4_kernel<4><<<g4, 256, 0, st>>>(p);
+        return static_cast<int>(cudaGetLastError());
+    }
     const int E = mode == DD_U8 ? 1 : (mode == DD_U16 ? 2 : 4);
     const int TC = 128 / E;
     const int NL = VW * (4 / E), TJ = NL > 8 ? 16 : 32;

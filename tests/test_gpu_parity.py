@@ -394,6 +394,30 @@ def test_u4_packed_input_matches_oracle(B, oracle, case, monkeypatch):
         plan.destroy()
 
 
+@pytest.mark.parametrize("shape", [(256, 4096), (130, 5002), (38, 1000), (2, 300), (600, 3000)])
+def test_u4_time_major_matches_oracle(B, oracle, shape, monkeypatch):
+    """Packed 4-bit delivered time-major ([nsamps][nchans/2], even channel in the low nibble,
+    reading R16) through dd_execute_tm and the chunked dd_execute_host_tm."""
+    import torch
+    nchans, nsamps = shape
+    rng = np.random.default_rng([nchans, nsamps, 44])
+    x8 = rng.integers(0, 16, (nchans, nsamps), dtype=np.uint8)
+    xp_cm = W.pack_u4(x8)                                             # oracle input: packed along time
+    x_tm = np.ascontiguousarray(x8.T)                                 # [nsamps][nchans]
+    xp_tm = (x_tm[:, 0::2] | (x_tm[:, 1::2] << 4)).astype(np.uint8)   # packed along channels
+    dms = np.arange(7) * 9.0
+    with B.Plan(nchans, nsamps, 1500.0, -200.0 / nchans, 64e-6, dms, B.DD_U4) as plan:
+        ref = oracle.dedisperse_u4(xp_cm, plan.shift_table(), plan.out_len)
+        d_out = torch.full((plan.ndm, plan.out_len), -7, dtype=torch.int32, device="cuda")
+        plan.execute_tm(torch.from_numpy(xp_tm).cuda(), d_out)
+        torch.cuda.synchronize()
+        assert np.array_equal(d_out.cpu().numpy().view(np.uint32), ref)
+        monkeypatch.setenv("DD_HOST_CHUNKS", "3")
+        h_out = torch.full((plan.ndm, plan.out_len), -7, dtype=torch.int32).pin_memory()
+        plan.execute_host_tm(torch.from_numpy(xp_tm).pin_memory(), h_out)
+        assert np.array_equal(h_out.numpy().view(np.uint32), ref)
+
+
 def test_u4_all_fifteen_and_errors(B):
     import torch
     nchans, nsamps = 1031, 2000
