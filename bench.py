@@ -204,8 +204,13 @@ def run_ours(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
     torch.cuda.set_device(local_rank)
+    # stdout carries exactly ONE JSON line: anything libraries print (NCCL's version banner) goes
+    # to stderr until the line is written
+    sys.stdout.flush()
+    saved_stdout = os.dup(1)
+    os.dup2(2, 1)
     dist = None
-    if world > 1:
+    if world > 1 or "TORCHELASTIC_RUN_ID" in os.environ:  # under torch.distributed.run, also at N = 1
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     from paper_2311_05341_b200 import binding as B, build, shard
@@ -411,7 +416,9 @@ def run_ours(args):
                     "api": "dd_execute_host (pinned host buffers)", "checksum": checksum},
             "gpu_launches": args.steps * plan.info("LAUNCHES"),
             "clocks": clocks}
-    print(json.dumps(line))
+    sys.stdout.flush()
+    os.dup2(saved_stdout, 1)
+    print(json.dumps(line), flush=True)
     plan.destroy()
     if dist is not None:
         dist.barrier()
