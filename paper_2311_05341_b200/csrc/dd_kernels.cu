@@ -69,13 +69,36 @@ __device__ __forceinline__ uint32_t odd_bytes(uint32_t w)
     return __byte_perm(w, 0u, 0x4341);
 }
 
+// ------------------------------------------------------------------ tensor-memory scratch (FM = 4)
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr)
+        : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16])
+{
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+        :
+        : "r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
+          "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+        : "memory");
+}
+
 // ------------------------------------------------------------------ per-mode accumulators
 template <int MODE, int FM>
 struct Acc;
 
 // FM (u8 only) = which adds are issued as IMAD (x * one + acc, `one` a runtime 1 that ptxas
 // cannot fold) on the fma pipe instead of IADD3 on the alu pipe:
-//   0 none; 1 W += x (both words); 2 O += odd(x) (both words)
+//   0 none; 1 W += x (both words); 2 O += odd(x) (both words);
+//   4 = 2, and the four uint32 flush accumulators per word live in tensor memory instead of
+//       registers (TMEM is lane-private scratch here: a thread reads and writes only its own lane)
 template <int FM>
 struct Acc<DD_U8, FM> {
     uint32_t W = 0, O = 0;           // packed, flushed every <= 256 channels
@@ -88,7 +111,7 @@ struct Acc<DD_U8, FM> {
         } else {
             W = W + x + y;
         }
-        if (FM == 2) {
+        if (FM == 2 || FM == 4) {
             O = odd_bytes(x) * one + O;
             O = odd_bytes(y) * one + O;
         } else {
@@ -217,7 +240,19 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    constexpr bool TMEM = MODE == DD_U8 && FM == 4;
+    constexpr int NCOL = 4 * RD * RJ * VW;  // TMEM columns per consumer thread (4 uint32 per word)
+    static_assert(!TMEM || (NCOL % 16 == 0 && (NCW + 3) / 4 * NCOL <= 512), "TMEM scratch layout");
+    if (TMEM && warp == 0) {  // one warp allocates all 512 columns (one CTA per SM: always granted)
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(bar_full + 960u) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
     __syncthreads();
+    uint32_t tmem = 0;
+    if (TMEM) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem) : "r"(bar_full + 960u) : "memory");
+    }
 
     if (warp == NCW) {
         // ===================== producer warp: lane l stages slot l of each stage
@@ -251,6 +286,7 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
                 phase ^= 1u;
             }
         }
+        if (TMEM) asm volatile("bar.sync 1, %0;" ::"r"((NCW + 1) * 32) : "memory");  // TMEM is freed after the consumers
         return;
     }
 
@@ -262,6 +298,12 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
     const uint32_t lane_byte = static_cast<uint32_t>((wj * RJ * 32 + lane) * S);
     const uint32_t stage_u32 = smem_u32(stage0);
 
+    // FM = 4: this thread's 4 uint32 accumulators per word sit in its own TMEM lane, columns
+    // [(warp / 4) * NCOL, +NCOL) of lane quarter warp % 4 (the hardware's rule: warp w of a CTA
+    // reaches lanes 32 * (w % 4) .. +31); column ((r*RJ + i)*VW + v)*4 + l.  Touched only at a
+    // flush (every 256 channels) and at the end, 16 columns per instruction.
+    const uint32_t taddr = tmem + (static_cast<uint32_t>((warp & 3) * 32) << 16) + static_cast<uint32_t>((warp >> 2) * NCOL);
+    bool parked = false;  // TMEM holds valid partial sums
     int s = 0;
     int since_flush = 0;
     uint32_t phase = 0;
@@ -307,12 +349,42 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
         since_flush += CH;
         if (Acc<MODE, FM>::kNeedsFlush && since_flush + CH > 256) {
             since_flush = 0;
+            if constexpr (TMEM) {
+                if (k + 1 < p.nk) {  // (the last stage's sums go straight to the epilogue)
 #pragma unroll
-            for (int r = 0; r < RD; ++r)
+                    for (int ch = 0; ch < NCOL / 16; ++ch) {
+                        uint32_t t[16];
+                        if (parked) {
+                            tmem_ld16(taddr + ch * 16, t);
+                        } else {
 #pragma unroll
-                for (int i = 0; i < RJ; ++i)
+                            for (int q = 0; q < 16; ++q) t[q] = 0u;
+                        }
 #pragma unroll
-                    for (int v = 0; v < VW; ++v) acc[r][i][v].flush();
+                        for (int q = 0; q < 4; ++q) {
+                            const int wi = ch * 4 + q;
+                            Acc<MODE, FM> &a = acc[wi / (RJ * VW)][(wi / VW) % RJ][wi % VW];
+                            const uint32_t E = a.W - (a.O << 8);
+                            t[q * 4 + 0] += E & 0xFFFFu;
+                            t[q * 4 + 1] += a.O & 0xFFFFu;
+                            t[q * 4 + 2] += E >> 16;
+                            t[q * 4 + 3] += a.O >> 16;
+                            a.W = 0;
+                            a.O = 0;
+                        }
+                        tmem_st16(taddr + ch * 16, t);
+                    }
+                    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+                    parked = true;
+                }
+            } else {
+#pragma unroll
+                for (int r = 0; r < RD; ++r)
+#pragma unroll
+                    for (int i = 0; i < RJ; ++i)
+#pragma unroll
+                        for (int v = 0; v < VW; ++v) acc[r][i][v].flush();
+            }
         }
         if (++s == nstage) {
             s = 0;
@@ -321,6 +393,41 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
     }
 
     // ========================= store (a7): lane l of superword j is output sample l*L + j
+    if constexpr (TMEM) {
+#pragma unroll
+        for (int ch = 0; ch < NCOL / 16; ++ch) {
+            uint32_t t[16];
+            if (parked) {
+                tmem_ld16(taddr + ch * 16, t);
+            } else {
+#pragma unroll
+                for (int q = 0; q < 16; ++q) t[q] = 0u;
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int wi = ch * 4 + q;
+                const int r = wi / (RJ * VW), i = (wi / VW) % RJ, v = wi % VW;
+                const Acc<MODE, FM> &a = acc[r][i][v];
+                const uint32_t E = a.W - (a.O << 8);
+                const uint32_t val[4] = {t[q * 4 + 0] + (E & 0xFFFFu), t[q * 4 + 1] + (a.O & 0xFFFFu),
+                                         t[q * 4 + 2] + (E >> 16), t[q * 4 + 3] + (a.O >> 16)};
+                const int d = b * D_DM + wd * RD + r;
+                const int64_t j = j0 + (wj * RJ + i) * 32 + lane;
+                if (d < p.ndm && j < p.L) {
+                    uint32_t *o = static_cast<uint32_t *>(p.out) + static_cast<size_t>(d) * p.out_pitch;
+#pragma unroll
+                    for (int l = 0; l < 4; ++l) {
+                        const int64_t tt = static_cast<int64_t>(v * 4 + l) * p.L + j;
+                        if (tt < p.out_len) o[tt] = val[l];
+                    }
+                }
+            }
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        asm volatile("bar.sync 1, %0;" ::"r"((NCW + 1) * 32) : "memory");
+        if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
+        return;
+    }
 #pragma unroll
     for (int r = 0; r < RD; ++r) {
         const int d = b * D_DM + wd * RD + r;
@@ -939,18 +1046,19 @@ struct Variant {
 // first with TUNE == 0 whose shared-memory ring fits (smaller DM blocks = shorter staged
 // windows; smaller CH = smaller stages).  TUNE == 1 entries are reachable through the
 // DD_FORCE_VARIANT environment variable only (A/B measurements, profiles/).
-// u8: LDS.64 superwords, 12 DM warps x 6 superwords, odd-lane adds on the fma pipe (FM = 2):
-// the r01 sweep (profiles/r01_tuning.md) measured 58.0 ms on the headline config against
-// 68.3 ms for the LDS.32 / 16-warp / all-alu shape (entry 7).
+// u8: LDS.64 superwords, 12 DM warps x 12 superwords, odd-lane adds on the fma pipe and the
+// uint32 flush accumulators parked in tensor memory (FM = 4): 56.4 ms on the headline config
+// against 58.4 ms with the accumulators in registers (entry 6: 6 superwords per thread) and
+// 68.3 ms for the LDS.32 / 16-warp / all-alu first shape (entry 7); profiles/r01_tuning.md.
 const Variant kVariants[] = {
     //         mode  VW RD RJ  WD  WJ  CH FM NB OW tune
-    DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 2, 1, 4, 0),   // 0
-    DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 16, 2, 1, 4, 0),   // 1
-    DD_VARIANT(DD_U8, 2, 1, 6, 6, 2, 16, 2, 1, 4, 0),    // 2
-    DD_VARIANT(DD_U8, 2, 1, 6, 6, 2, 8, 2, 1, 4, 0),     // 3
-    DD_VARIANT(DD_U8, 2, 1, 6, 3, 4, 8, 2, 1, 4, 0),     // 4
-    DD_VARIANT(DD_U8, 2, 1, 6, 3, 4, 4, 2, 1, 4, 0),     // 5
-    DD_VARIANT(DD_U8, 2, 1, 6, 1, 12, 4, 2, 1, 4, 0),    // 6  one DM per block: always fits
+    DD_VARIANT(DD_U8, 2, 1, 12, 12, 1, 16, 4, 1, 4, 0),  // 0
+    DD_VARIANT(DD_U8, 2, 1, 12, 12, 1, 8, 4, 1, 4, 0),   // 1
+    DD_VARIANT(DD_U8, 2, 1, 12, 6, 2, 8, 4, 1, 4, 0),    // 2
+    DD_VARIANT(DD_U8, 2, 1, 12, 3, 4, 4, 4, 1, 4, 0),    // 3
+    DD_VARIANT(DD_U8, 2, 1, 6, 3, 4, 4, 4, 1, 4, 0),     // 4
+    DD_VARIANT(DD_U8, 2, 1, 6, 1, 12, 4, 4, 1, 4, 0),    // 5  one DM per block: always fits
+    DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 2, 1, 4, 1),   // 6  r01b shape: accumulators in registers (A/B only)
     DD_VARIANT(DD_U8, 1, 1, 8, 16, 1, 16, 0, 1, 4, 1),   // 7  r01 first shape (A/B only)
     DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 1, 1, 4, 1),   // 8  W on fma instead of O (A/B only)
     DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 0, 1, 4, 1),   // 9  all adds on alu (A/B only)
