@@ -434,11 +434,23 @@ static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void 
     int G = 0;
     edge[0] = 0;
     const char *env = std::getenv("DD_HOST_CHUNKS");  // explicit request (tests, tuning): n equal chunks
-    if (!env && plan->out_len >= 64 * tile) {
+    if (!env && plan->out_len >= 32 * tile) {
         // Tapered schedule: only the first chunk's host->device copy (chunk + max_shift halo) and
         // the last chunk's device->host copy are exposed, so those two chunks are small; in
         // between a chunk may grow as long as its copy hides behind the previous chunk's kernels.
-        static const double frac[dd_plan::kHostChunks] = {0.04, 0.07, 0.12, 0.20, 0.25, 0.20, 0.09, 0.03};
+        double frac[dd_plan::kHostChunks] = {0.04, 0.07, 0.12, 0.20, 0.25, 0.20, 0.09, 0.03};
+        if (const char *fe = std::getenv("DD_HOST_FRAC")) {  // tuning aid: 8 comma-separated fractions
+            double v[dd_plan::kHostChunks];
+            int n = 0;
+            for (const char *q = fe; n < dd_plan::kHostChunks && *q; ++n) {
+                char *end = nullptr;
+                v[n] = std::strtod(q, &end);
+                if (end == q) break;
+                q = *end == ',' ? end + 1 : end;
+            }
+            if (n == dd_plan::kHostChunks)
+                for (int g = 0; g < n; ++g) frac[g] = v[g];
+        }
         double cum = 0.0;
         for (int g = 0; g < dd_plan::kHostChunks; ++g) {
             cum += frac[g];
