@@ -369,7 +369,7 @@ def run_ours(args):
     smem_alg_bytes = adds * smem_b                      # one sample read from shared memory per add
     hbm_alg_bytes = int(cfg.nchans * cfg.nsamps * in_b) + plan.ndm * plan.out_len * 4
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "r01b_traffic.csv")  # from the ncu captures (r01b_summary.md)
+    tpath = os.path.join(ROOT, "profiles", "r01b_traffic.csv")  # from the ncu captures (r01b/r01d summaries)
     if os.path.exists(tpath) and not args.nsamps:
         with open(tpath) as f:
             for ln in f.read().splitlines()[1:]:
@@ -382,7 +382,7 @@ def run_ours(args):
     roofline = {"bound": "smem", "kernel": "dedisperse_kernel",
                 "achieved": smem_alg_bytes / main_s / 1e9, "peak": smem_peak_gbs, "unit": "GB/s",
                 "frac": smem_alg_bytes / main_s / 1e9 / smem_peak_gbs, "traffic": traffic,
-                "traffic_note": "DRAM bytes per launch (ncu, profiles/r01b_summary.md); algorithmic HBM bytes %d"
+                "traffic_note": "DRAM bytes per launch (ncu, profiles/r01d_summary.md for u8, r01b_summary.md for u16/f32); algorithmic HBM bytes %d"
                                 % hbm_alg_bytes,
                 "peak_kind": "derived (paper Eq. 8): %d SMs x %d B/clk x %.0f MHz (%s sm_max_mhz)"
                              % (N_SM, SMEM_BYTES_PER_SM_CLK, sm_max_mhz, peak_kind),
