@@ -456,7 +456,7 @@ static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void 
             cum += frac[g];
             int64_t e = g + 1 == dd_plan::kHostChunks
                             ? plan->out_len
-                            : static_cast<int64_t>(cum * static_cast<double>(plan->out_len)) / unit * unit;
+                            : static_cast<int64_t>(cum * static_cast<double>(plan->out_len)) / tile * tile;  // whole j tiles
             if (e > edge[G]) edge[++G] = e;
         }
     } else {
@@ -467,7 +467,9 @@ static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void 
         }
         if (want > dd_plan::kHostChunks) want = dd_plan::kHostChunks;
         if (want < 1) want = 1;
-        const int64_t C = ((plan->out_len + want - 1) / want + unit - 1) / unit * unit;
+        // whole j tiles per chunk when the block is long enough, else the alignment unit
+        const int64_t q = plan->out_len >= 4 * want * tile ? tile : unit;
+        const int64_t C = ((plan->out_len + want - 1) / want + q - 1) / q * q;
         while (edge[G] < plan->out_len) {
             const int64_t e = edge[G] + C < plan->out_len ? edge[G] + C : plan->out_len;
             edge[++G] = e;
