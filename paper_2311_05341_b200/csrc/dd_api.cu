@@ -26,8 +26,10 @@ struct dd_plan {
     void *d_in_own = nullptr, *d_out_own = nullptr;
     static constexpr int kHostChunks = 8;
     bool host_made = false;
-    cudaStream_t st_h2d = nullptr, st_d2h = nullptr;
-    cudaEvent_t ev_in[kHostChunks + 1] = {}, ev_done[kHostChunks + 1] = {};
+    cudaStream_t st_h2d = nullptr, st_d2h = nullptr, st_pre = nullptr;
+    cudaEvent_t ev_in[kHostChunks + 1] = {}, ev_done[kHostChunks + 1] = {}, ev_pre[kHostChunks + 1] = {};
+    uint32_t *d_X2 = nullptr;  // second chunk workspace: chunk g+1 is interleaved while chunk g is dedispersed
+    size_t x2_bytes = 0;
     // optional per-kernel timing (dd_plan_set_timing): ring of event triples
     static constexpr int kRing = 64;
     bool timing = false;
@@ -57,6 +59,7 @@ void free_device(dd_plan *p)
         cudaFree(p->d_X);
         cudaFree(p->d_ofs);
         cudaFree(p->d_blk);
+        cudaFree(p->d_X2);
         cudaFree(p->d_in_own);
         cudaFree(p->d_out_own);
         if (p->ev_made)
@@ -65,8 +68,10 @@ void free_device(dd_plan *p)
         if (p->host_made) {
             for (cudaEvent_t e : p->ev_in) cudaEventDestroy(e);
             for (cudaEvent_t e : p->ev_done) cudaEventDestroy(e);
+            for (cudaEvent_t e : p->ev_pre) cudaEventDestroy(e);
             cudaStreamDestroy(p->st_h2d);
             cudaStreamDestroy(p->st_d2h);
+            cudaStreamDestroy(p->st_pre);
         }
         if (cur >= 0 && cur != p->device) cudaSetDevice(cur);
     }
@@ -232,15 +237,13 @@ BlockGeom geom_for(const dd_plan *plan, int64_t out_len, int64_t nsamps)
     return g;
 }
 
-int launch_block(const dd_plan *plan, const BlockGeom &g, const void *d_in, int64_t in_pitch,
-                 void *d_out, int64_t out_pitch, cudaStream_t st, const cudaEvent_t *ev,
-                 bool time_major = false)
+int launch_prepass(const dd_plan *plan, const BlockGeom &g, const void *d_in, int64_t in_pitch,
+                   uint32_t *X, cudaStream_t st, bool time_major)
 {
     const dd::Tiling &t = plan->til;
-    if (ev) cudaEventRecord(ev[0], st);
     dd::InterleaveParams ip;
     ip.in = d_in;
-    ip.X = plan->d_X;
+    ip.X = X;
     ip.nsamps = g.nsamps;
     ip.in_pitch = in_pitch;
     ip.L = g.L;
@@ -250,12 +253,18 @@ int launch_block(const dd_plan *plan, const BlockGeom &g, const void *d_in, int6
     ip.j_begin = 0;
     ip.j_end = g.Lw;
     ip.nchunk = static_cast<int>((g.Lw + 1023) / 1024);
-    if ((time_major ? dd::launch_interleave_tm(plan->in_dtype, t.shape.VW, ip, st)
-                    : dd::launch_interleave(plan->in_dtype, t.shape.VW, ip, st)) != 0)
-        return DD_ERR_CUDA;
-    if (ev) cudaEventRecord(ev[1], st);
+    return (time_major ? dd::launch_interleave_tm(plan->in_dtype, t.shape.VW, ip, st)
+                       : dd::launch_interleave(plan->in_dtype, t.shape.VW, ip, st)) != 0
+               ? DD_ERR_CUDA
+               : DD_OK;
+}
+
+int launch_main(const dd_plan *plan, const BlockGeom &g, const uint32_t *X, void *d_out,
+                int64_t out_pitch, cudaStream_t st)
+{
+    const dd::Tiling &t = plan->til;
     dd::KernelParams kp;
-    kp.X = plan->d_X;
+    kp.X = X;
     kp.ofs = plan->d_ofs;
     kp.blk = plan->d_blk;
     kp.out = d_out;
@@ -274,8 +283,20 @@ int launch_block(const dd_plan *plan, const BlockGeom &g, const void *d_in, int6
     kp.stage_bytes = t.rows_bytes + t.shape.D_DM() * t.shape.CH * t.shape.OW;
     kp.one = 1u;
     const int grid = t.ndb * g.ntj;
-    if (dd::launch_dedisperse(t.variant, kp, grid, static_cast<int>(t.smem_bytes), st) != 0)
-        return DD_ERR_CUDA;
+    return dd::launch_dedisperse(t.variant, kp, grid, static_cast<int>(t.smem_bytes), st) != 0 ? DD_ERR_CUDA
+                                                                                                : DD_OK;
+}
+
+int launch_block(const dd_plan *plan, const BlockGeom &g, const void *d_in, int64_t in_pitch,
+                 void *d_out, int64_t out_pitch, cudaStream_t st, const cudaEvent_t *ev,
+                 bool time_major = false)
+{
+    if (ev) cudaEventRecord(ev[0], st);
+    int rc = launch_prepass(plan, g, d_in, in_pitch, plan->d_X, st, time_major);
+    if (rc != DD_OK) return rc;
+    if (ev) cudaEventRecord(ev[1], st);
+    rc = launch_main(plan, g, plan->d_X, d_out, out_pitch, st);
+    if (rc != DD_OK) return rc;
     if (ev) cudaEventRecord(ev[2], st);
     return DD_OK;
 }
@@ -416,10 +437,12 @@ static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void 
     }
     if (!plan->host_made) {
         if (cudaStreamCreateWithFlags(&plan->st_h2d, cudaStreamNonBlocking) != cudaSuccess ||
-            cudaStreamCreateWithFlags(&plan->st_d2h, cudaStreamNonBlocking) != cudaSuccess)
+            cudaStreamCreateWithFlags(&plan->st_d2h, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaStreamCreateWithFlags(&plan->st_pre, cudaStreamNonBlocking) != cudaSuccess)
             return DD_ERR_CUDA;
         for (int g = 0; g <= dd_plan::kHostChunks; ++g)
             if (cudaEventCreateWithFlags(&plan->ev_in[g], cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&plan->ev_pre[g], cudaEventDisableTiming) != cudaSuccess ||
                 cudaEventCreateWithFlags(&plan->ev_done[g], cudaEventDisableTiming) != cudaSuccess)
                 return DD_ERR_CUDA;
         plan->host_made = true;
@@ -483,6 +506,25 @@ static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void 
     const size_t in_pitch = sample_bytes(dt, plan->nsamps);
     const size_t out_pitch = static_cast<size_t>(plan->out_len) * 4;
 
+    // second workspace, large enough for the longest chunk
+    {
+        size_t need_x = 0;
+        for (int g = 0; g < G; ++g) {
+            const BlockGeom bg = geom_for(plan, edge[g + 1] - edge[g], edge[g + 1] - edge[g] + plan->max_shift);
+            const size_t b = static_cast<size_t>(t.nch_pad) * bg.Lw * t.shape.sw_bytes();
+            if (b > need_x) need_x = b;
+        }
+        if (G > 1 && need_x > plan->x2_bytes) {
+            cudaFree(plan->d_X2);
+            plan->d_X2 = nullptr;
+            plan->x2_bytes = 0;
+            if (cudaMalloc(reinterpret_cast<void **>(&plan->d_X2), need_x) != cudaSuccess) {
+                cudaGetLastError();
+                return DD_ERR_ALLOC;
+            }
+            plan->x2_bytes = need_x;
+        }
+    }
     // the copy stream starts after whatever the caller has queued on `st`
     if (cudaEventRecord(plan->ev_done[G], st) != cudaSuccess) return DD_ERR_CUDA;
     cudaStreamWaitEvent(plan->st_h2d, plan->ev_done[G], 0);
@@ -506,12 +548,20 @@ static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void 
             have = need_c;
         }
         cudaEventRecord(plan->ev_in[g], plan->st_h2d);
-        cudaStreamWaitEvent(st, plan->ev_in[g], 0);
+        // pre-pass of chunk g on its own stream into workspace g & 1, as soon as its input has
+        // arrived and the main kernel of chunk g-2 (the previous user of that workspace) is done:
+        // it overlaps the main kernel of chunk g-1 (HBM-bound next to a shared-memory-bound kernel)
         const BlockGeom bg = geom_for(plan, o1 - o0, need - o0);
-        const int rc = tm ? launch_block(plan, bg, din + o0 * sample_bytes(dt, plan->nchans), plan->nchans,
-                                         dout + o0 * 4, plan->out_len, st, nullptr, true)
-                          : launch_block(plan, bg, din + sample_bytes(dt, o0), plan->nsamps, dout + o0 * 4,
-                                         plan->out_len, st, nullptr);
+        uint32_t *Xg = (g & 1) ? plan->d_X2 : plan->d_X;
+        cudaStreamWaitEvent(plan->st_pre, plan->ev_in[g], 0);
+        if (g >= 2) cudaStreamWaitEvent(plan->st_pre, plan->ev_done[g - 2], 0);
+        int rc = tm ? launch_prepass(plan, bg, din + o0 * sample_bytes(dt, plan->nchans), plan->nchans, Xg,
+                                     plan->st_pre, true)
+                    : launch_prepass(plan, bg, din + sample_bytes(dt, o0), plan->nsamps, Xg, plan->st_pre, false);
+        if (rc != DD_OK) return rc;
+        cudaEventRecord(plan->ev_pre[g], plan->st_pre);
+        cudaStreamWaitEvent(st, plan->ev_pre[g], 0);
+        rc = launch_main(plan, bg, Xg, dout + o0 * 4, plan->out_len, st);
         if (rc != DD_OK) return rc;
         cudaEventRecord(plan->ev_done[g], st);
         cudaStreamWaitEvent(plan->st_d2h, plan->ev_done[g], 0);
