@@ -1,19 +1,22 @@
-// dd_kernels.cu -- sm_100a kernels of libdd.so (SURVEY.md 8(a) rows a3-a7).
+// dd_kernels.cu -- sm_100a kernels of libdd.so (SURVEY.md 8(a) rows a3-a7 and 8(f) rows).
 //
 // Two kernels per dd_execute:
-//   1. interleave_kernel: in[c][t] (u8/u16/f32) -> X[c][j] (32-bit words), lane k of word j
-//      holding in[c][k*L + j].  HBM-bound, ~2x the input size of traffic.
-//   2. dedisperse_kernel: the shifted sum.  A thread block owns D_DM DM trials x D_J words of
-//      the interleaved time axis.  A producer warp streams channel rows into a ring of
-//      shared-memory stages with cp.async.bulk (TMA 1-D, mbarrier complete_tx); consumer
-//      warps read one 32-bit word per lane at the (DM, channel) word offset -- conflict-free
-//      for ANY shift -- and accumulate LANES samples per word:
+//   1. interleave_kernel (interleave_tm_kernel for time-major input): in[c][t] (u4/u8/u16/f32)
+//      -> X[c][j], superwords of VW 32-bit words, lane l of superword j holding in[c][l*L + j].
+//      HBM-bound.
+//   2. dedisperse_kernel: the shifted sum.  A thread block owns D_DM DM trials x D_J
+//      superwords of the interleaved time axis.  A producer warp streams channel windows into
+//      a ring of shared-memory stages with cp.async.bulk (TMA 1-D, mbarrier complete_tx);
+//      consumer warps read one superword per lane (LDS.32/64/128) at the (DM, channel) offset
+//      -- aligned and conflict-free for ANY shift -- and accumulate all its lanes at once:
 //        u8 : W += w (carries run across byte lanes), O += odd bytes of w as two 16-bit
-//             lanes (PRMT); even lanes are recovered as W - 256*O at the flush, every
-//             256 channels (exact: 257*255 < 2^16), into four uint32 accumulators;
+//             lanes (PRMT, the add as IMAD on the fma pipe); even lanes are recovered as
+//             W - 256*O at the flush, after at most 256 channels (256*255 < 2^16), into four
+//             uint32 accumulators per word that live in tensor memory (lane-private scratch);
 //        u16: W += w, H += w >> 16; low lane recovered as W - 65536*H at the end;
 //        f32: FADD.
-// No tensor cores: a shifted-diagonal sum is not a contraction.
+// Also here: transpose_kernel (dd_transpose), bin_time_*_kernel (dd_bin_time).
+// The tensor cores' MMA units are not used: a shifted-diagonal sum is not a contraction.
 #include <cuda_runtime.h>
 
 #include <cstdint>
