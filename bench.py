@@ -14,6 +14,13 @@ collective; value = units of all ranks / max-over-ranks time ("scaling": "weak")
 
 --impl reference: the CPU oracle (oracle/dedisp_oracle.c), as it stands, timed on the host
 cores on a bounded sample of the same workload (a subset of DM rows per step).
+
+Besides the contract's keys the line carries: `e2e` (dd_execute_host, pinned host buffers, copies
+inside the timed region), `roofline` (shared-memory pipe, the binding one) with `roofline_alu` and
+`roofline_hbm`, `cpu_baseline` (the oracle on the host cores, about 10 s), `kernels_ms`,
+`realtime_factor` (Eq. 10), `time_major` (dd_execute_tm / dd_execute_host_tm / dd_transpose) and
+`time_binning` (dd_bin_time).  Extra workloads: headline_u4 (packed 4-bit), paper52 (the paper's
+section 5.2 plan); --nsamps overrides the block length.
 """
 from __future__ import annotations
 
