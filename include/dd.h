@@ -139,7 +139,8 @@ int dd_bin_time(const void *d_in, void *d_out, int nchans, int64_t nsamps, int f
 /*
  * The same transform with HOST buffers: h_in [nchans][nsamps], h_out [ndm][out_len].
  * Pipelined over up to 8 time chunks (default: a tapered 8-chunk schedule with a small first
- * and last chunk; environment variable DD_HOST_CHUNKS=<n> asks for n equal chunks): chunk g's input range [o0, o1 + max_shift) of every channel is copied to a
+ * and last chunk; environment variable DD_HOST_CHUNKS=<n> asks for n equal chunks,
+ * DD_HOST_FRAC=<8 comma-separated fractions> replaces the tapered schedule -- tuning aids): chunk g's input range [o0, o1 + max_shift) of every channel is copied to a
  * plan-owned device buffer on a copy stream while chunk g-1 runs through the kernels (pre-pass
  * on a plan-owned stream, main kernel on `cuda_stream`) and chunk g-2's output columns are
  * copied back on a second copy stream.
