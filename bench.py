@@ -162,17 +162,53 @@ def time_oracle(cfg, steps: int, warmup: int, rows_per_step: int | None = None, 
                       % (nrows, cfg.ndm, cfg.nchans, steps, dt)}, dt / steps
 
 
+def time_tiled(cfg, x, budget_s: float = 10.0):
+    """cpu_baseline_tiled: the paper's tiled OpenMP CPU kernel (Algorithm 2, PAPER.md:91-141;
+    cpu_tiled/) on a bounded sample of the workload -- a contiguous block of DM rows (its DM tiles
+    share cache lines only between neighbouring trials), full out_len, all channels.  Tile sizes:
+    the fastest of cpu_tiled.tiled.CANDIDATES on a short sub-sample (the paper autotunes them per
+    CPU and plan).  8-bit input only, as in the paper."""
+    if cfg.in_dtype != W.U8:
+        return None
+    from cpu_tiled import tiled
+    from oracle import oracle   # only its shift table: the tiled kernel takes shifts as an input
+    tiled.build()
+    threads = tiled.omp_threads()
+    table, mx = oracle.shift_table(cfg.nchans, cfg.f_high, cfg.chan_bw, cfg.tsamp, cfg.dm_list)
+    out_len = cfg.nsamps - mx
+    d0 = (cfg.ndm // 2) // 64 * 64
+    per_row = float(out_len) * cfg.nchans
+    probe_rows = int(min(cfg.ndm - d0, max(64, 2 * threads)))
+    best, best_rate = None, 0.0
+    for tile in tiled.CANDIDATES:
+        t0 = time.perf_counter()
+        tiled.dedisperse_u8(x, table[d0:d0 + probe_rows], out_len, tile)
+        rate = probe_rows * per_row / (time.perf_counter() - t0)
+        if rate > best_rate:
+            best, best_rate = tile, rate
+    rows = int(min(cfg.ndm - d0, max(probe_rows, budget_s * best_rate / per_row)))
+    t0 = time.perf_counter()
+    tiled.dedisperse_u8(x, table[d0:d0 + rows], out_len, best)
+    dt = time.perf_counter() - t0
+    return {"value": rows * per_row / dt, "unit": UNIT, "cores": threads,
+            "kind": "paper Algorithm 2 (tiled OpenMP + SIMD CPU kernel, cpu_tiled/)",
+            "tile": {"D_t": best[0], "D_dm": best[1], "D_f": best[2], "acc16": best[3]},
+            "sample": "DM rows %d..%d of %d x full out_len x all %d channels, %.1f s"
+                      % (d0, d0 + rows, cfg.ndm, cfg.nchans, dt)}
+
+
 def run_reference(args):
     rank, _, world = _dist_env()
     if rank != 0:
         return 0
     cfg = W.ALL_CONFIGS[args.config]
     base, ms = time_oracle(cfg, args.steps, args.warmup)
+    from oracle import oracle
     line = {"impl": "reference", "metric": METRIC, "value": base["value"], "unit": UNIT,
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": _dtype_name(cfg), "data": "synthetic",
-            "config": _config_dict(cfg, None), "cpu_baseline": base,
+            "config": _config_dict(cfg, _OracleFacts(cfg, oracle)), "cpu_baseline": base,
             "e2e": {"value": base["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -186,6 +222,15 @@ def _dtype_name(cfg):
             W.U4: "u4 in (widened to u8 lanes by the pre-pass), packed u16/u32 integer accumulate, u32 out"}[cfg.in_dtype]
 
 
+class _OracleFacts:
+    """out_len / max_shift / ndm of a config from the ORACLE's shift table, for the reference
+    arm's `config` (same keys and values as our arm's, which takes them from the plan)."""
+
+    def __init__(self, cfg, oracle):
+        _, mx = oracle.shift_table(cfg.nchans, cfg.f_high, cfg.chan_bw, cfg.tsamp, cfg.dm_list)
+        self.max_shift, self.out_len, self.ndm = mx, cfg.nsamps - mx, cfg.ndm
+
+
 def _config_dict(cfg, plan):
     d = {"workload": cfg.name + ("" if cfg.nsamps == W.ALL_CONFIGS_NSAMPS.get(cfg.name, cfg.nsamps)
                                  else " (nsamps overridden)"), "nchans": cfg.nchans, "nsamps": cfg.nsamps, "ndm": cfg.ndm,
@@ -193,15 +238,47 @@ def _config_dict(cfg, plan):
          "tsamp_s": cfg.tsamp, "in_dtype": W.DTYPE_NAME[cfg.in_dtype],
          "l2": "input (%.2f GiB) and output are each larger than the 126 MB L2; no flush needed"
                % (cfg.nchans * cfg.nsamps * W.ELEM_BYTES[cfg.in_dtype] / 2 ** 30)}
-    if plan is not None:
-        d.update({"out_len": plan.out_len, "max_shift": plan.max_shift,
-                  "adds_per_step": plan.ndm * plan.out_len * cfg.nchans,
-                  "adds_nominal": cfg.ndm * cfg.nsamps * cfg.nchans,
-                  "tile": "D_DM=%d x D_J=%d superwords x %d lanes, CH=%d, %d stages, %d B smem, grid %d x %d threads"
-                          % (plan.info("D_DM"), plan.info("D_J"), plan.info("LANES"), plan.info("CH"),
-                             plan.info("NSTAGE"), plan.info("SMEM_BYTES"), plan.info("GRID"),
-                             plan.info("THREADS"))})
+    d.update({"out_len": plan.out_len, "max_shift": plan.max_shift,
+              "adds_per_step": plan.ndm * plan.out_len * cfg.nchans,
+              "adds_nominal": cfg.ndm * cfg.nsamps * cfg.nchans})
     return d
+
+
+def _tile_string(plan):
+    return ("D_DM=%d x D_J=%d superwords x %d lanes, CH=%d, %d stages, %d B smem, grid %d x %d threads"
+            % (plan.info("D_DM"), plan.info("D_J"), plan.info("LANES"), plan.info("CH"),
+               plan.info("NSTAGE"), plan.info("SMEM_BYTES"), plan.info("GRID"), plan.info("THREADS")))
+
+
+# ------------------------------------------------------------------------- measured on-chip peaks
+PROBE_UNITS = {"SM_COUNT": "SMs", "SM_CLOCK_MHZ": "MHz", "LDS32": "B/clk/SM", "LDS64": "B/clk/SM",
+               "LDS128": "B/clk/SM", "TMEM_LD": "B/clk/SM", "TMEM_LD_WITH_LDS": "B/clk/SM (each of TMEM and LDS.64)"}
+
+
+def measure_peaks(B):
+    """Every dd_probe key -> value (lane-instructions or bytes per clock per SM, SM clock, SM count)."""
+    return {k: B.probe(k) for k in B.PROBES}
+
+
+def run_probe_peaks(args):
+    """--probe-peaks: run the library's on-chip probes (include/dd.h dd_probe) and print them as one
+    JSON line: the measured denominators of `roofline` / `roofline_alu`."""
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
+    from paper_2311_05341_b200 import binding as B, build
+    build.build()
+    p = measure_peaks(B)
+    nsm, mhz = p["SM_COUNT"], p["SM_CLOCK_MHZ"]
+    line = {"probe": "dd_probe", "device": torch.cuda.get_device_name(0),
+            "per_clk_per_sm": {k: v for k, v in p.items() if k not in ("SM_COUNT", "SM_CLOCK_MHZ")},
+            "units": {k: PROBE_UNITS.get(k, "lane-instructions/clk/SM") for k in p},
+            "sm_count": nsm, "sm_clock_mhz": mhz,
+            "smem_read_peak_gbs": max(p["LDS32"], p["LDS64"], p["LDS128"]) * nsm * mhz * 1e6 / 1e9,
+            "int_add_peak_tlane_s": p["IADD3"] * nsm * mhz * 1e6 / 1e12,
+            "fp32_add_peak_tlane_s": p["FADD"] * nsm * mhz * 1e6 / 1e12}
+    print(json.dumps(line))
+    return 0
 
 
 # ------------------------------------------------------------------------- our arm
@@ -229,6 +306,7 @@ def run_ours(args):
 
     cfg = W.ALL_CONFIGS[args.config]
     hbm_gbs, sm_max_mhz, peak_kind = _peaks()
+    probed = measure_peaks(B) if rank == 0 else None   # before the timed region: a second of GPU time
     plan = B.Plan(cfg.nchans, cfg.nsamps, cfg.f_high, cfg.chan_bw, cfg.tsamp, cfg.dm_list, cfg.in_dtype)
     table = plan.shift_table() if cfg.npulses else None
     # every rank: its own block (seed offset by rank), resident in HBM before timing starts
@@ -287,7 +365,13 @@ def run_ours(args):
     ms_e2e /= e2e_steps
     h2d = h_in.numel() * h_in.element_size()
     d2h = h_out.numel() * h_out.element_size()
-    checksum = int(h_out.view(torch.int32)[:, ::4097].to(torch.int64).sum().item())
+    # the timed host path must reproduce the device-resident plane bit for bit (same kernels, same
+    # per-output summation order -- float32 too); tests/ tie that plane to the oracle
+    plan.execute(x, out)
+    torch.cuda.synchronize()
+    e2e_verified = bool(torch.equal(h_out, out.cpu()))
+    if not e2e_verified:
+        raise SystemExit("bench.py: dd_execute_host output differs from dd_execute output")
 
     # ---- time-major input: transpose pre-step + the same path
     tm = None
@@ -368,15 +452,22 @@ def run_ours(args):
     main_s = float(np.mean(main_ms)) * 1e-3
     il_s = float(np.mean(il_ms)) * 1e-3
     kadds = adds / main_s
-    clk = sm_max_mhz * 1e6
-    int_peak = N_SM * INT_LANES_PER_SM_CLK * clk
-    smem_peak_gbs = N_SM * SMEM_BYTES_PER_SM_CLK * clk / 1e9
+    # measured on this device by the library's own probes (dd_probe): bytes per clock per SM read
+    # from shared memory (best of LDS.32/.64/.128), IADD3 lane-instructions per clock per SM, and
+    # the SM clock during the probes; the derived figures (paper Eq. 8) are reported beside them
+    n_sm = int(probed["SM_COUNT"])
+    clk = probed["SM_CLOCK_MHZ"] * 1e6
+    smem_b_clk = max(probed["LDS32"], probed["LDS64"], probed["LDS128"])
+    int_peak = n_sm * probed["IADD3"] * clk
+    smem_peak_gbs = n_sm * smem_b_clk * clk / 1e9
+    smem_peak_derived = N_SM * SMEM_BYTES_PER_SM_CLK * sm_max_mhz * 1e6 / 1e9
+    int_peak_derived = N_SM * INT_LANES_PER_SM_CLK * sm_max_mhz * 1e6
     in_b = W.ELEM_BYTES[cfg.in_dtype]
     smem_b = 1 if cfg.in_dtype == W.U4 else in_b        # 4-bit samples travel as bytes on chip
     smem_alg_bytes = adds * smem_b                      # one sample read from shared memory per add
     hbm_alg_bytes = int(cfg.nchans * cfg.nsamps * in_b) + plan.ndm * plan.out_len * 4
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "r01b_traffic.csv")  # from the ncu captures (r01b/r01d summaries)
+    tpath = os.path.join(ROOT, "profiles", "r02_traffic.csv")  # dram bytes per launch from the committed ncu captures
     if os.path.exists(tpath) and not args.nsamps:
         with open(tpath) as f:
             for ln in f.read().splitlines()[1:]:
@@ -391,14 +482,14 @@ def run_ours(args):
                 "frac": smem_alg_bytes / main_s / 1e9 / smem_peak_gbs, "traffic": traffic,
                 "traffic_note": "DRAM bytes per launch (ncu, profiles/r01d_summary.md for u8, r01b_summary.md for u16/f32); algorithmic HBM bytes %d"
                                 % hbm_alg_bytes,
-                "peak_kind": "derived (paper Eq. 8): %d SMs x %d B/clk x %.0f MHz (%s sm_max_mhz)"
-                             % (N_SM, SMEM_BYTES_PER_SM_CLK, sm_max_mhz, peak_kind),
+                "peak_kind": "measured (dd_probe): %.1f B/clk/SM x %d SMs x %.0f MHz; derived (paper Eq. 8) %.0f GB/s"
+                             % (smem_b_clk, n_sm, probed["SM_CLOCK_MHZ"], smem_peak_derived),
                 "algorithmic_bytes_per_add": smem_b, "adds_per_launch": adds,
                 "kernel_ms": main_s * 1e3, "share_of_step": share}
     roofline_alu = {"bound": "alu", "achieved": kadds / 1e12, "peak": int_peak / 1e12, "unit": "Tadd/s",
                     "frac": kadds / int_peak,
-                    "peak_kind": "derived: %d SMs x %d INT32 add lanes/clk x %.0f MHz"
-                                 % (N_SM, INT_LANES_PER_SM_CLK, sm_max_mhz),
+                    "peak_kind": "measured (dd_probe): %.1f IADD3 lanes/clk/SM x %d SMs x %.0f MHz; derived %.2f Tadd/s"
+                                 % (probed["IADD3"], n_sm, probed["SM_CLOCK_MHZ"], int_peak_derived / 1e12),
                     "note": "sample-adds against one-add-per-lane integer peak (BASELINE.json's metric); "
                             "a packed add performs 4 (u8) / 2 (u16) sample-adds, so frac may exceed 1"}
     roofline_hbm = {"bound": "hbm", "achieved": hbm_alg_bytes / (ms_step * 1e-3) / 1e9, "peak": hbm_gbs,
@@ -406,21 +497,25 @@ def run_ours(args):
                     "peak_kind": peak_kind + " copy bandwidth",
                     "staged_l2_to_smem_bytes": plan.info("STAGE_BYTES")}
 
-    cpu_base, _ = time_oracle(cfg, 1, 1, x=h_in.numpy() if cfg.in_dtype != W.U16
-                              else h_in.view(torch.int16).numpy().view(np.uint16))
+    x_host = h_in.numpy() if cfg.in_dtype != W.U16 else h_in.view(torch.int16).numpy().view(np.uint16)
+    cpu_base, _ = time_oracle(cfg, 1, 1, x=x_host)
+    cpu_tiled = time_tiled(cfg, x_host)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": _dtype_name(cfg),
-            "data": "synthetic", "config": _config_dict(cfg, plan),
+            "data": "synthetic", "config": _config_dict(cfg, plan), "tile": _tile_string(plan),
             "realtime_factor": {"t_obs_over_t": cfg.nsamps * cfg.tsamp / (ms_step * 1e-3),
                                 "out_len_tsamp_over_t": plan.out_len * cfg.tsamp / (ms_step * 1e-3)},
             "value_nominal": world * cfg.ndm * cfg.nsamps * cfg.nchans / (ms_step * 1e-3),
             "kernels_ms": {"interleave_kernel": il_s * 1e3, "dedisperse_kernel": main_s * 1e3},
             "roofline": roofline, "roofline_alu": roofline_alu, "roofline_hbm": roofline_hbm,
-            "cpu_baseline": cpu_base, "time_major": tm, "time_binning": binning,
+            "measured_peaks": probed,
+            "cpu_baseline": cpu_base, "cpu_baseline_tiled": cpu_tiled,
+            "time_major": tm, "time_binning": binning,
             "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e,
                     "steps": e2e_steps, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "api": "dd_execute_host (pinned host buffers)", "checksum": checksum},
+                    "api": "dd_execute_host (pinned host buffers, default chunk schedule)",
+                    "e2e_verified": e2e_verified},
             "gpu_launches": args.steps * plan.info("LAUNCHES"),
             "clocks": clocks}
     sys.stdout.flush()
@@ -448,6 +543,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="headline", choices=list(W.ALL_CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--probe-peaks", action="store_true",
+                    help="only run the library's on-chip peak probes (dd_probe) and print them")
     ap.add_argument("--nsamps", type=int, default=0,
                     help="override the config's block length (sanity check: adds/s should not depend "
                          "on the observation length, PAPER.md:287); the line's config says so")
@@ -455,6 +552,8 @@ def main():
     _apply_overrides(args)
     if args.impl == "reference":
         return run_reference(args)
+    if args.probe_peaks:
+        return run_probe_peaks(args)
     return run_ours(args)
 
 

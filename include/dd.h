@@ -68,9 +68,8 @@ int dd_shift_table_build(int nchans, double f_high_MHz, double chan_bw_MHz, doub
  * nsamps <= 0, unknown dtype); DD_ERR_SHIFT_TOO_LARGE (max shift >= nsamps);
  * DD_ERR_OVERFLOW (u8: 255*nchans >= 2^32; u16: 65535*nchans >= 2^32; u4: 15*nchans >= 2^32); DD_ERR_ALLOC;
  * DD_ERR_CUDA; DD_ERR_UNSUPPORTED_DEVICE; DD_ERR_UNSUPPORTED_PLAN.
- * Tuning aid: if the environment variable DD_FORCE_VARIANT=<n> is set, entry n of the
- * compiled kernel table (dd_kernels.cu) is used instead of the automatic choice; the
- * results are identical, only the tiling differs (A/B measurements under profiles/).
+ * The library reads no environment variable.  (A tuning build, `build.py --tuning`, adds the A/B
+ * kernel shapes of profiles/r01_tuning.md and honours DD_FORCE_VARIANT=<n>; never the default.)
  */
 int dd_plan_create(dd_plan **out, int nchans, int64_t nsamps, double f_high_MHz,
                    double chan_bw_MHz, double tsamp_s, const double *dm_list, int ndm,
@@ -138,16 +137,20 @@ int dd_bin_time(const void *d_in, void *d_out, int nchans, int64_t nsamps, int f
 
 /*
  * The same transform with HOST buffers: h_in [nchans][nsamps], h_out [ndm][out_len].
- * Pipelined over up to 8 time chunks (default: a tapered 8-chunk schedule with a small first
- * and last chunk; environment variable DD_HOST_CHUNKS=<n> asks for n equal chunks,
- * DD_HOST_FRAC=<8 comma-separated fractions> replaces the tapered schedule -- tuning aids): chunk g's input range [o0, o1 + max_shift) of every channel is copied to a
- * plan-owned device buffer on a copy stream while chunk g-1 runs through the kernels (pre-pass
- * on a plan-owned stream, main kernel on `cuda_stream`) and chunk g-2's output columns are
- * copied back on a second copy stream.
+ * Pipelined over up to 8 time chunks (the time sharding of SURVEY.md 8(e) inside one GPU): chunk g =
+ * output samples [o0, o1) of every DM trial from input samples [o0, o1 + max_shift) of every
+ * channel.  Default schedule: 8 tapered chunks (4, 7, 12, 20, 25, 20, 9, 3 % of the output, edges on
+ * whole j tiles) when the block has at least 32 j tiles, else up to 6 equal chunks of at least 8 j
+ * tiles; dd_plan_set_host_chunks overrides it.  A chunk's new input samples are copied to a
+ * plan-owned device buffer on a copy stream while the previous chunk runs through the kernels
+ * (pre-pass on a plan-owned stream; main kernels alternate between `cuda_stream` and a second
+ * plan-owned stream so that consecutive chunks overlap at their partial last waves) and the chunk
+ * before that is copied back on a second copy stream.
  * Returns after the last copy has finished.  Buffers should be page-locked for full PCIe
- * bandwidth and true overlap (pageable memory works, slower).  The device buffers, two
- * streams and the events are created on first use and kept until dd_plan_destroy.
- * Errors as dd_execute, plus DD_ERR_ALLOC.
+ * bandwidth and true overlap (pageable memory works, slower).  The device buffers, streams and
+ * events are created on first use and kept until dd_plan_destroy.
+ * Errors as dd_execute, plus DD_ERR_ALLOC.  On an error after work has been queued the call
+ * drains every stream it used before returning, so the caller's buffers are quiescent.
  */
 int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream);
 
@@ -158,6 +161,12 @@ int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_str
  * fused time-major pre-pass of dd_execute_tm.  Errors as dd_execute_host and dd_execute_tm.
  */
 int dd_execute_host_tm(dd_plan *plan, const void *h_in_tm, void *h_out, void *cuda_stream);
+
+/*
+ * Chunk count of dd_execute_host / dd_execute_host_tm for this plan: 0 = the default schedule
+ * described above, 1..8 = that many equal chunks (1 = no pipelining).  DD_ERR_INVALID_ARG otherwise.
+ */
+int dd_plan_set_host_chunks(dd_plan *plan, int nchunks);
 
 /*
  * Facts about the plan, for tests and the benchmark.  `what` is one of DD_INFO_*; unknown
@@ -190,6 +199,46 @@ int64_t dd_plan_info(const dd_plan *plan, int what);
  */
 int dd_plan_set_timing(dd_plan *plan, int on);
 int dd_plan_kernel_times(dd_plan *plan, int max_n, float *interleave_ms, float *main_ms);
+
+/*
+ * Measured on-chip peaks of the current device: the denominators of the benchmark's rooflines.
+ * The paper derives them from data-sheet numbers (shared-memory bandwidth = 4 B x banks x clock x
+ * SMs, Eq. 8; arithmetic peak, Eq. 9); this call measures them with small
+ * register-only / shared-memory-only kernels, one 1024-thread CTA per SM (dd_probe.cu).
+ * `what` is one of DD_PROBE_*; *value receives
+ *   DD_PROBE_SM_COUNT            number of SMs
+ *   DD_PROBE_SM_CLOCK_MHZ        SM clock during a probe kernel (cycle counter / CUDA-event time)
+ *   DD_PROBE_LDS32/64/128        shared-memory bytes read per clock per SM with LDS.32/.64/.128
+ *   DD_PROBE_IADD3 ... _SHF      lane-instructions per clock per SM of that instruction
+ *                                (IADD3 = three-input integer add; VIADD16X2 = packed 2 x 16-bit add;
+ *                                IMAD = 32-bit multiply-add, fma pipe; SHIFT_ADD = acc + (x >> k),
+ *                                SASS LEA.HI; IMAD_HI = high half multiply-add; IDP4A = 4-way byte dot
+ *                                product; LOP3, PRMT, SHF, FADD as named)
+ *   DD_PROBE_TMEM_LD             tensor-memory bytes read per clock per SM (tcgen05.ld.32x32b.x8)
+ *   DD_PROBE_TMEM_LD_WITH_LDS    the same while the CTA also reads as many bytes with LDS.64
+ * Blocking (synchronises the device); allocates and frees a few MB.  Errors: DD_ERR_INVALID_ARG,
+ * DD_ERR_UNSUPPORTED_DEVICE, DD_ERR_ALLOC, DD_ERR_CUDA.
+ */
+enum {
+    DD_PROBE_SM_COUNT = 0,
+    DD_PROBE_SM_CLOCK_MHZ = 1,
+    DD_PROBE_LDS32 = 2,
+    DD_PROBE_LDS64 = 3,
+    DD_PROBE_LDS128 = 4,
+    DD_PROBE_IADD3 = 5,
+    DD_PROBE_VIADD16X2 = 6,
+    DD_PROBE_IMAD = 7,
+    DD_PROBE_FADD = 8,
+    DD_PROBE_LOP3 = 9,
+    DD_PROBE_PRMT = 10,
+    DD_PROBE_SHIFT_ADD = 11,
+    DD_PROBE_IMAD_HI = 12,
+    DD_PROBE_IDP4A = 13,
+    DD_PROBE_SHF = 14,
+    DD_PROBE_TMEM_LD = 15,
+    DD_PROBE_TMEM_LD_WITH_LDS = 16
+};
+int dd_probe(int what, double *value);
 
 /* Frees everything the plan owns (waits for the device first).  NULL is a no-op. */
 void dd_plan_destroy(dd_plan *plan);

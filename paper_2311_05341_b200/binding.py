@@ -28,8 +28,14 @@ INFO = {"D_DM": 0, "D_J": 1, "LANES": 2, "L": 3, "SMEM_BYTES": 4, "GRID": 5, "TH
 
 # every symbol include/dd.h declares (tests check the .so exports all of them)
 SYMBOLS = ("dd_shift_table_build", "dd_plan_create", "dd_plan_shift_table", "dd_execute",
-           "dd_execute_host", "dd_execute_host_tm", "dd_execute_tm", "dd_transpose", "dd_bin_time", "dd_plan_info", "dd_plan_set_timing", "dd_plan_kernel_times",
-           "dd_plan_destroy", "dd_strerror", "dd_version")
+           "dd_execute_host", "dd_execute_host_tm", "dd_execute_tm", "dd_transpose", "dd_bin_time",
+           "dd_plan_set_host_chunks", "dd_plan_info", "dd_plan_set_timing", "dd_plan_kernel_times",
+           "dd_probe", "dd_plan_destroy", "dd_strerror", "dd_version")
+
+# dd_probe keys (include/dd.h DD_PROBE_*)
+PROBES = {"SM_COUNT": 0, "SM_CLOCK_MHZ": 1, "LDS32": 2, "LDS64": 3, "LDS128": 4, "IADD3": 5,
+          "VIADD16X2": 6, "IMAD": 7, "FADD": 8, "LOP3": 9, "PRMT": 10, "SHIFT_ADD": 11, "IMAD_HI": 12,
+          "IDP4A": 13, "SHF": 14, "TMEM_LD": 15, "TMEM_LD_WITH_LDS": 16}
 
 _lib = None
 
@@ -70,12 +76,16 @@ def lib() -> ctypes.CDLL:
         L.dd_bin_time.argtypes = [c.c_void_p, c.c_void_p, c.c_int, c.c_int64, c.c_int, c.c_int, c.c_void_p]
         L.dd_transpose.restype = c.c_int
         L.dd_transpose.argtypes = [c.c_void_p, c.c_void_p, c.c_int, c.c_int64, c.c_int, c.c_void_p]
+        L.dd_plan_set_host_chunks.restype = c.c_int
+        L.dd_plan_set_host_chunks.argtypes = [c.c_void_p, c.c_int]
         L.dd_plan_info.restype = c.c_int64
         L.dd_plan_info.argtypes = [c.c_void_p, c.c_int]
         L.dd_plan_set_timing.restype = c.c_int
         L.dd_plan_set_timing.argtypes = [c.c_void_p, c.c_int]
         L.dd_plan_kernel_times.restype = c.c_int
         L.dd_plan_kernel_times.argtypes = [c.c_void_p, c.c_int, c.c_void_p, c.c_void_p]
+        L.dd_probe.restype = c.c_int
+        L.dd_probe.argtypes = [c.c_int, c.POINTER(c.c_double)]
         L.dd_plan_destroy.restype = None
         L.dd_plan_destroy.argtypes = [c.c_void_p]
         L.dd_strerror.restype = c.c_char_p
@@ -92,6 +102,15 @@ def strerror(status: int) -> str:
 
 def version() -> str:
     return lib().dd_version().decode()
+
+
+def probe(what: str) -> float:
+    """dd_probe: one measured on-chip peak of the current device (keys of PROBES)."""
+    v = ctypes.c_double(0.0)
+    rc = lib().dd_probe(PROBES[what], ctypes.byref(v))
+    if rc != DD_OK:
+        raise DDError(rc, "dd_probe(%s)" % what)
+    return float(v.value)
 
 
 def _dm_array(dm_list) -> np.ndarray:
@@ -187,6 +206,13 @@ class Plan:
         rc = lib().dd_execute_host_tm(self._h, _host_ptr(h_in_tm), _host_ptr(h_out), _stream_ptr(stream))
         if rc != DD_OK:
             raise DDError(rc, "dd_execute_host_tm")
+
+    # -- dd_plan_set_host_chunks
+    def set_host_chunks(self, nchunks: int) -> None:
+        """0 = the default schedule of dd_execute_host, 1..8 = that many equal chunks."""
+        rc = lib().dd_plan_set_host_chunks(self._h, int(nchunks))
+        if rc != DD_OK:
+            raise DDError(rc, "dd_plan_set_host_chunks")
 
     # -- dd_plan_set_timing / dd_plan_kernel_times
     def set_timing(self, on: bool) -> None:

@@ -1,6 +1,9 @@
 """Build libdd.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
-    python -m paper_2311_05341_b200.build [--force] [--verbose]
+    python -m paper_2311_05341_b200.build [--force] [--verbose] [--tuning]
+
+--tuning adds -DDD_TUNING: the A/B kernel shapes of profiles/r01_tuning.md and the
+DD_FORCE_VARIANT environment variable exist only in such a build (never the default).
 
 The .so is git-ignored and travels to the GPU box with the gpurun snapshot.
 """
@@ -15,7 +18,7 @@ _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(_ROOT, "include")
 LIB = os.path.join(_HERE, "libdd.so")
-SOURCES = ["dd_host.cpp", "dd_kernels.cu", "dd_api.cu"]
+SOURCES = ["dd_host.cpp", "dd_kernels.cu", "dd_api.cu", "dd_probe.cu"]
 HEADERS = [os.path.join(CSRC, "dd_internal.h"), os.path.join(INCLUDE, "dd.h")]
 
 NVCC_FLAGS = [
@@ -42,11 +45,13 @@ def needs_build() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not needs_build():
+def build(force: bool = False, verbose: bool = False, tuning: bool = False) -> str:
+    if not force and not tuning and not needs_build():
         return LIB
     tmp = LIB + ".tmp.%d" % os.getpid()
     cmd = [_nvcc()] + NVCC_FLAGS + ["-I", INCLUDE, "-I", CSRC]
+    if tuning:
+        cmd += ["-DDD_TUNING"]
     if verbose:
         cmd += ["-Xptxas", "-v"]
     cmd += [os.path.join(CSRC, s) for s in SOURCES] + ["-o", tmp]
@@ -62,4 +67,4 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, tuning="--tuning" in sys.argv))

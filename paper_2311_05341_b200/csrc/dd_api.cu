@@ -26,7 +26,8 @@ struct dd_plan {
     void *d_in_own = nullptr, *d_out_own = nullptr;
     static constexpr int kHostChunks = 8;
     bool host_made = false;
-    cudaStream_t st_h2d = nullptr, st_d2h = nullptr, st_pre = nullptr;
+    int host_chunks = 0;  // dd_plan_set_host_chunks: 0 = default tapered schedule, n = n equal chunks
+    cudaStream_t st_h2d = nullptr, st_d2h = nullptr, st_pre = nullptr, st_main2 = nullptr;
     cudaEvent_t ev_in[kHostChunks + 1] = {}, ev_done[kHostChunks + 1] = {}, ev_pre[kHostChunks + 1] = {};
     uint32_t *d_X2 = nullptr;  // second chunk workspace: chunk g+1 is interleaved while chunk g is dedispersed
     size_t x2_bytes = 0;
@@ -72,6 +73,7 @@ void free_device(dd_plan *p)
             cudaStreamDestroy(p->st_h2d);
             cudaStreamDestroy(p->st_d2h);
             cudaStreamDestroy(p->st_pre);
+            cudaStreamDestroy(p->st_main2);
         }
         if (cur >= 0 && cur != p->device) cudaSetDevice(cur);
     }
@@ -154,8 +156,12 @@ int dd_plan_create(dd_plan **out, int nchans, int64_t nsamps, double f_high_MHz,
 
         // first compiled variant of this dtype whose shared-memory ring fits
         bool found = false;
-        const char *force = std::getenv("DD_FORCE_VARIANT");  // tuning experiments only
+#ifdef DD_TUNING
+        const char *force = std::getenv("DD_FORCE_VARIANT");  // tuning builds only (build.py --tuning)
         const int forced = force ? std::atoi(force) : -1;
+#else
+        const int forced = -1;
+#endif
         for (int v = 0; v < dd::num_variants() && !found; ++v) {
             const dd::KernelShape &sh = dd::variant_shape(v);
             if (sh.mode != kernel_mode(in_dtype)) continue;
@@ -416,6 +422,88 @@ int dd_execute_host_tm(dd_plan *plan, const void *h_in_tm, void *h_out, void *cu
     return execute_host_impl(plan, h_in_tm, h_out, cuda_stream, true);
 }
 
+// Streams and events of the host-buffer path, created on first use: all of them or none.
+static int make_host_objects(dd_plan *plan)
+{
+    if (plan->host_made) return DD_OK;
+    constexpr int NE = dd_plan::kHostChunks + 1;
+    cudaStream_t s[4] = {};
+    cudaEvent_t e[3 * NE] = {};
+    bool ok = true;
+    for (cudaStream_t &x : s) ok = ok && cudaStreamCreateWithFlags(&x, cudaStreamNonBlocking) == cudaSuccess;
+    for (cudaEvent_t &x : e) ok = ok && cudaEventCreateWithFlags(&x, cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) {
+        for (cudaStream_t x : s)
+            if (x) cudaStreamDestroy(x);
+        for (cudaEvent_t x : e)
+            if (x) cudaEventDestroy(x);
+        cudaGetLastError();
+        return DD_ERR_CUDA;
+    }
+    plan->st_h2d = s[0];
+    plan->st_d2h = s[1];
+    plan->st_pre = s[2];
+    plan->st_main2 = s[3];
+    for (int g = 0; g < NE; ++g) {
+        plan->ev_in[g] = e[g];
+        plan->ev_pre[g] = e[NE + g];
+        plan->ev_done[g] = e[2 * NE + g];
+    }
+    plan->host_made = true;
+    return DD_OK;
+}
+
+// Chunk edges of the host-buffer path: chunk g = output samples [edge[g], edge[g+1]).  Returns
+// the number of chunks (1 .. kHostChunks).  Chunk lengths are whole j tiles when the block is
+// long enough, else a multiple of 16 samples per lane (keeps every chunk's rows as aligned as
+// the caller's).
+static int host_schedule(const dd_plan *plan, int64_t *edge)
+{
+    const dd::Tiling &t = plan->til;
+    const int NL = t.shape.lanes();
+    const int64_t tile = static_cast<int64_t>(NL) * t.shape.D_J();
+    const int64_t unit = static_cast<int64_t>(NL) * 16;
+    int G = 0;
+    edge[0] = 0;
+    if (plan->host_chunks == 0 && plan->out_len >= 32 * tile) {
+        // Tapered schedule: only the first chunk's host->device copy (chunk + max_shift halo) and
+        // the last chunk's device->host copy are exposed, so those two chunks are small; in
+        // between a chunk may grow as long as its copy hides behind the previous chunk's kernels.
+        static const double frac[dd_plan::kHostChunks] = {0.04, 0.07, 0.12, 0.20, 0.25, 0.20, 0.09, 0.03};
+        double cum = 0.0;
+        for (int g = 0; g < dd_plan::kHostChunks; ++g) {
+            cum += frac[g];
+            int64_t e = g + 1 == dd_plan::kHostChunks
+                            ? plan->out_len
+                            : static_cast<int64_t>(cum * static_cast<double>(plan->out_len)) / tile * tile;
+            if (e > plan->out_len) e = plan->out_len;
+            if (e > edge[G]) edge[++G] = e;
+        }
+        return G;
+    }
+    int want = plan->host_chunks ? plan->host_chunks : 6;
+    if (!plan->host_chunks) {  // at least 8 j tiles per chunk so that the grid still fills the GPU
+        const int64_t by_tiles = plan->out_len / (8 * tile);
+        if (want > by_tiles) want = static_cast<int>(by_tiles);
+    }
+    if (want > dd_plan::kHostChunks) want = dd_plan::kHostChunks;
+    if (want < 1) want = 1;
+    const int64_t q = plan->out_len >= 4 * want * tile ? tile : unit;
+    const int64_t C = ((plan->out_len + want - 1) / want + q - 1) / q * q;
+    while (edge[G] < plan->out_len) {
+        const int64_t e = edge[G] + C < plan->out_len ? edge[G] + C : plan->out_len;
+        edge[++G] = e;
+    }
+    return G;
+}
+
+int dd_plan_set_host_chunks(dd_plan *plan, int nchunks)
+{
+    if (!plan || nchunks < 0 || nchunks > dd_plan::kHostChunks) return DD_ERR_INVALID_ARG;
+    plan->host_chunks = nchunks;
+    return DD_OK;
+}
+
 // tm: the host block is time-major [nsamps][nchans]; a chunk's new samples are then ONE contiguous
 // range of it (a plain 1-D copy) and the chunk runs through the fused time-major pre-pass.
 static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream, bool tm)
@@ -435,69 +523,10 @@ static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void 
         plan->d_out_own = nullptr;
         return DD_ERR_ALLOC;
     }
-    if (!plan->host_made) {
-        if (cudaStreamCreateWithFlags(&plan->st_h2d, cudaStreamNonBlocking) != cudaSuccess ||
-            cudaStreamCreateWithFlags(&plan->st_d2h, cudaStreamNonBlocking) != cudaSuccess ||
-            cudaStreamCreateWithFlags(&plan->st_pre, cudaStreamNonBlocking) != cudaSuccess)
-            return DD_ERR_CUDA;
-        for (int g = 0; g <= dd_plan::kHostChunks; ++g)
-            if (cudaEventCreateWithFlags(&plan->ev_in[g], cudaEventDisableTiming) != cudaSuccess ||
-                cudaEventCreateWithFlags(&plan->ev_pre[g], cudaEventDisableTiming) != cudaSuccess ||
-                cudaEventCreateWithFlags(&plan->ev_done[g], cudaEventDisableTiming) != cudaSuccess)
-                return DD_ERR_CUDA;
-        plan->host_made = true;
-    }
+    if (const int rc = make_host_objects(plan); rc != DD_OK) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    // chunk length: a multiple of 16 samples per lane (keeps every chunk's rows as aligned as the
-    // caller's), at least 8 j tiles per chunk so that the grid still fills the GPU
-    const int NL = t.shape.lanes();
-    const int64_t tile = static_cast<int64_t>(NL) * t.shape.D_J();
-    const int64_t unit = static_cast<int64_t>(NL) * 16;
     int64_t edge[dd_plan::kHostChunks + 1];  // chunk g = output samples [edge[g], edge[g+1])
-    int G = 0;
-    edge[0] = 0;
-    const char *env = std::getenv("DD_HOST_CHUNKS");  // explicit request (tests, tuning): n equal chunks
-    if (!env && plan->out_len >= 32 * tile) {
-        // Tapered schedule: only the first chunk's host->device copy (chunk + max_shift halo) and
-        // the last chunk's device->host copy are exposed, so those two chunks are small; in
-        // between a chunk may grow as long as its copy hides behind the previous chunk's kernels.
-        double frac[dd_plan::kHostChunks] = {0.04, 0.07, 0.12, 0.20, 0.25, 0.20, 0.09, 0.03};
-        if (const char *fe = std::getenv("DD_HOST_FRAC")) {  // tuning aid: 8 comma-separated fractions
-            double v[dd_plan::kHostChunks];
-            int n = 0;
-            for (const char *q = fe; n < dd_plan::kHostChunks && *q; ++n) {
-                char *end = nullptr;
-                v[n] = std::strtod(q, &end);
-                if (end == q) break;
-                q = *end == ',' ? end + 1 : end;
-            }
-            if (n == dd_plan::kHostChunks)
-                for (int g = 0; g < n; ++g) frac[g] = v[g];
-        }
-        double cum = 0.0;
-        for (int g = 0; g < dd_plan::kHostChunks; ++g) {
-            cum += frac[g];
-            int64_t e = g + 1 == dd_plan::kHostChunks
-                            ? plan->out_len
-                            : static_cast<int64_t>(cum * static_cast<double>(plan->out_len)) / tile * tile;  // whole j tiles
-            if (e > edge[G]) edge[++G] = e;
-        }
-    } else {
-        int want = env ? std::atoi(env) : 6;
-        if (!env) {
-            const int64_t by_tiles = plan->out_len / (8 * tile);
-            if (want > by_tiles) want = static_cast<int>(by_tiles);
-        }
-        if (want > dd_plan::kHostChunks) want = dd_plan::kHostChunks;
-        if (want < 1) want = 1;
-        // whole j tiles per chunk when the block is long enough, else the alignment unit
-        const int64_t q = plan->out_len >= 4 * want * tile ? tile : unit;
-        const int64_t C = ((plan->out_len + want - 1) / want + q - 1) / q * q;
-        while (edge[G] < plan->out_len) {
-            const int64_t e = edge[G] + C < plan->out_len ? edge[G] + C : plan->out_len;
-            edge[++G] = e;
-        }
-    }
+    const int G = host_schedule(plan, edge);
 
     const unsigned char *hin = static_cast<const unsigned char *>(h_in);
     unsigned char *din = static_cast<unsigned char *>(plan->d_in_own);
@@ -525,9 +554,21 @@ static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void 
             plan->x2_bytes = need_x;
         }
     }
-    // the copy stream starts after whatever the caller has queued on `st`
+    // Nothing has been queued so far.  From here on a failure must not return while copies or
+    // kernels that touch the caller's buffers are still in flight: drain every stream first.
+    auto fail = [&](int rc) {
+        cudaStreamSynchronize(plan->st_h2d);
+        cudaStreamSynchronize(plan->st_pre);
+        cudaStreamSynchronize(plan->st_main2);
+        cudaStreamSynchronize(st);
+        cudaStreamSynchronize(plan->st_d2h);
+        cudaGetLastError();
+        return rc;
+    };
+    // the plan's streams start after whatever the caller has queued on `st`
     if (cudaEventRecord(plan->ev_done[G], st) != cudaSuccess) return DD_ERR_CUDA;
     cudaStreamWaitEvent(plan->st_h2d, plan->ev_done[G], 0);
+    cudaStreamWaitEvent(plan->st_main2, plan->ev_done[G], 0);
     int64_t have = 0;  // input samples [0, have) of every channel are on their way to the device
     for (int g = 0; g < G; ++g) {
         const int64_t o0 = edge[g], o1 = edge[g + 1];
@@ -544,7 +585,7 @@ static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void 
                                        in_pitch, sample_bytes(dt, need_c - have), plan->nchans,
                                        cudaMemcpyHostToDevice, plan->st_h2d);
             }
-            if (ce != cudaSuccess) return DD_ERR_CUDA;
+            if (ce != cudaSuccess) return fail(DD_ERR_CUDA);
             have = need_c;
         }
         cudaEventRecord(plan->ev_in[g], plan->st_h2d);
@@ -558,20 +599,25 @@ static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void 
         int rc = tm ? launch_prepass(plan, bg, din + o0 * sample_bytes(dt, plan->nchans), plan->nchans, Xg,
                                      plan->st_pre, true)
                     : launch_prepass(plan, bg, din + sample_bytes(dt, o0), plan->nsamps, Xg, plan->st_pre, false);
-        if (rc != DD_OK) return rc;
+        if (rc != DD_OK) return fail(rc);
         cudaEventRecord(plan->ev_pre[g], plan->st_pre);
-        cudaStreamWaitEvent(st, plan->ev_pre[g], 0);
-        rc = launch_main(plan, bg, Xg, dout + o0 * 4, plan->out_len, st);
-        if (rc != DD_OK) return rc;
-        cudaEventRecord(plan->ev_done[g], st);
+        // main kernels alternate between the caller's stream and a plan-owned one: chunks are
+        // independent, so the last partial wave of chunk g overlaps the first wave of chunk g+1
+        cudaStream_t sm = (g & 1) ? plan->st_main2 : st;
+        cudaStreamWaitEvent(sm, plan->ev_pre[g], 0);
+        rc = launch_main(plan, bg, Xg, dout + o0 * 4, plan->out_len, sm);
+        if (rc != DD_OK) return fail(rc);
+        cudaEventRecord(plan->ev_done[g], sm);
         cudaStreamWaitEvent(plan->st_d2h, plan->ev_done[g], 0);
         if (cudaMemcpy2DAsync(hout + o0 * 4, out_pitch, dout + o0 * 4, out_pitch,
                               static_cast<size_t>(o1 - o0) * 4, plan->ndm, cudaMemcpyDeviceToHost,
                               plan->st_d2h) != cudaSuccess)
-            return DD_ERR_CUDA;
+            return fail(DD_ERR_CUDA);
     }
-    if (cudaStreamSynchronize(plan->st_d2h) != cudaSuccess) return DD_ERR_CUDA;
-    if (cudaStreamSynchronize(st) != cudaSuccess) return DD_ERR_CUDA;
+    // every main kernel precedes a copy on st_d2h; the caller's stream also waits for the odd chunks
+    if (G > 1) cudaStreamWaitEvent(st, plan->ev_done[((G - 1) & 1) ? G - 1 : G - 2], 0);
+    if (cudaStreamSynchronize(plan->st_d2h) != cudaSuccess) return fail(DD_ERR_CUDA);
+    if (cudaStreamSynchronize(st) != cudaSuccess) return fail(DD_ERR_CUDA);
     return DD_OK;
 }
 

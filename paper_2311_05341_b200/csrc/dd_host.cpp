@@ -92,17 +92,19 @@ bool build_tiling(const KernelShape &shape, int variant, const int32_t *table, i
 
     const size_t nslot = static_cast<size_t>(t->ndb) * static_cast<size_t>(t->nch_pad);
     t->blk.assign(nslot * 4, 0);
-    int rows_bytes = 0;
+    // window sizes in int64: a coarse DM step times a long block can exceed int32, and such a
+    // stage must make this rung fail (next rung: smaller DM block), never wrap around
+    int64_t rows_bytes = 0;
     int64_t per_jtile_bytes = 0;
     for (int b = 0; b < t->ndb; ++b) {
         const int d0 = b * D_DM, d1 = std::min(ndm, d0 + D_DM);
         for (int k = 0; k < t->nk; ++k) {
-            int dst = 0;
+            int64_t dst = 0;
             for (int cl = 0; cl < CH; ++cl) {
                 const size_t slot = static_cast<size_t>(b) * t->nch_pad + static_cast<size_t>(k) * CH + cl;
                 const int c = t->chan[static_cast<size_t>(k) * CH + cl];
                 int32_t base = 0;
-                int sw = D_J;  // padding channel: a zero row of X, read at offset 0
+                int64_t sw = D_J;  // padding channel: a zero row of X, read at offset 0
                 if (c < nchans) {
                     int32_t lo = std::numeric_limits<int32_t>::max(), hi = 0;
                     for (int d = d0; d < d1; ++d) {
@@ -111,22 +113,23 @@ bool build_tiling(const KernelShape &shape, int variant, const int32_t *table, i
                         hi = std::max(hi, s);
                     }
                     base = lo - lo % A;
-                    sw = static_cast<int>(round_up(static_cast<int64_t>(D_J) + (hi - base), A));
+                    sw = round_up(static_cast<int64_t>(D_J) + (static_cast<int64_t>(hi) - base), A);
                 } else {
-                    sw = static_cast<int>(round_up(D_J, A));
+                    sw = round_up(D_J, A);
                 }
+                if (dst + sw * S > smem_limit) return false;  // this stage alone exceeds shared memory
                 int32_t *q = t->blk.data() + slot * 4;
                 q[0] = c;
                 q[1] = base;
-                q[2] = sw * S;
-                q[3] = dst;
+                q[2] = static_cast<int32_t>(sw * S);
+                q[3] = static_cast<int32_t>(dst);
                 dst += sw * S;
             }
             rows_bytes = std::max(rows_bytes, dst);
             per_jtile_bytes += dst;
         }
     }
-    t->rows_bytes = rows_bytes;
+    t->rows_bytes = static_cast<int>(rows_bytes);
     const int64_t ofs_stage_bytes = static_cast<int64_t>(D_DM) * CH * shape.OW;
     const int64_t stage_bytes = rows_bytes + ofs_stage_bytes;
     const int64_t barrier_bytes = 1024;  // mbarriers + slack, see dd_kernels.cu

@@ -246,8 +246,11 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
     constexpr bool TMEM = MODE == DD_U8 && FM == 4;
     constexpr int NCOL = 4 * RD * RJ * VW;  // TMEM columns per consumer thread (4 uint32 per word)
     static_assert(!TMEM || (NCOL % 16 == 0 && (NCW + 3) / 4 * NCOL <= 512), "TMEM scratch layout");
-    if (TMEM && warp == 0) {  // one warp allocates all 512 columns (one CTA per SM: always granted)
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(bar_full + 960u) : "memory");
+    // columns this shape needs, rounded up to the power of two >= 32 that tcgen05.alloc takes
+    constexpr int TNEED = (NCW + 3) / 4 * NCOL;
+    constexpr uint32_t TCOLS = TNEED <= 32 ? 32 : TNEED <= 64 ? 64 : TNEED <= 128 ? 128 : TNEED <= 256 ? 256 : 512;
+    if (TMEM && warp == 0) {  // one warp allocates (blocks until a co-resident TMEM user frees enough)
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(bar_full + 960u), "n"(TCOLS) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     __syncthreads();
@@ -428,7 +431,7 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
         }
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         asm volatile("bar.sync 1, %0;" ::"r"((NCW + 1) * 32) : "memory");
-        if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
+        if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(TCOLS) : "memory");
         return;
     }
 #pragma unroll
@@ -747,13 +750,10 @@ __global__ void __launch_bounds__(256) interleave_tm_kernel(const InterleavePara
         uint32_t w = 0u;
         if (t < p.nsamps) {
             const T *src = in + t * p.in_pitch + c0;  // in_pitch = nchans: elements per time row
-            if (false) {
-            } else {
 #pragma unroll
-                for (int k = 0; k < LPW; ++k) {
-                    const int c = c0 + lane * LPW + k;
-                    if (c < p.nchans) w |= static_cast<uint32_t>(src[lane * LPW + k]) << (8 * E * k);
-                }
+            for (int k = 0; k < LPW; ++k) {
+                const int c = c0 + lane * LPW + k;
+                if (c < p.nchans) w |= static_cast<uint32_t>(src[lane * LPW + k]) << (8 * E * k);
             }
         }
         tile[r][lane] = w;
@@ -1047,12 +1047,11 @@ struct Variant {
 
 // Ordered per mode from the largest DM block to the smallest; dd_plan_create takes the
 // first with TUNE == 0 whose shared-memory ring fits (smaller DM blocks = shorter staged
-// windows; smaller CH = smaller stages).  TUNE == 1 entries are reachable through the
-// DD_FORCE_VARIANT environment variable only (A/B measurements, profiles/).
+// windows; smaller CH = smaller stages).  The last rung of each mode (one DM trial per block)
+// always fits.  TUNE == 1 entries exist only in tuning builds (build.py --tuning, -DDD_TUNING)
+// and are reachable through the DD_FORCE_VARIANT environment variable of such a build.
 // u8: LDS.64 superwords, 12 DM warps x 12 superwords, odd-lane adds on the fma pipe and the
-// uint32 flush accumulators parked in tensor memory (FM = 4): 56.4 ms on the headline config
-// against 58.4 ms with the accumulators in registers (entry 6: 6 superwords per thread) and
-// 68.3 ms for the LDS.32 / 16-warp / all-alu first shape (entry 7); profiles/r01_tuning.md.
+// uint32 flush accumulators parked in tensor memory (FM = 4); profiles/r01_tuning.md.
 const Variant kVariants[] = {
     //         mode  VW RD RJ  WD  WJ  CH FM NB OW tune
     DD_VARIANT(DD_U8, 2, 1, 12, 12, 1, 16, 4, 1, 4, 0),  // 0
@@ -1061,22 +1060,24 @@ const Variant kVariants[] = {
     DD_VARIANT(DD_U8, 2, 1, 12, 3, 4, 4, 4, 1, 4, 0),    // 3
     DD_VARIANT(DD_U8, 2, 1, 6, 3, 4, 4, 4, 1, 4, 0),     // 4
     DD_VARIANT(DD_U8, 2, 1, 6, 1, 12, 4, 4, 1, 4, 0),    // 5  one DM per block: always fits
-    DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 2, 1, 4, 1),   // 6  r01b shape: accumulators in registers (A/B only)
-    DD_VARIANT(DD_U8, 1, 1, 8, 16, 1, 16, 0, 1, 4, 1),   // 7  r01 first shape (A/B only)
-    DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 1, 1, 4, 1),   // 8  W on fma instead of O (A/B only)
-    DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 0, 1, 4, 1),   // 9  all adds on alu (A/B only)
-    DD_VARIANT(DD_U16, 2, 1, 8, 16, 1, 16, 0, 1, 4, 0),  // 10 LDS.64, 16 words per offset fetch
-    DD_VARIANT(DD_U16, 1, 1, 8, 16, 1, 16, 0, 1, 4, 0),  // 11
-    DD_VARIANT(DD_U16, 1, 1, 8, 4, 4, 16, 0, 1, 4, 0),   // 12
-    DD_VARIANT(DD_U16, 1, 1, 8, 4, 4, 8, 0, 1, 4, 0),    // 13
-    DD_VARIANT(DD_U16, 1, 1, 8, 1, 16, 4, 0, 1, 4, 0),   // 14 one DM per block: always fits
-    DD_VARIANT(DD_U16, 1, 2, 8, 16, 1, 16, 0, 1, 4, 1),  // 15 r01b shape: 2 DMs x 8 words (A/B only)
-    DD_VARIANT(DD_F32, 1, 2, 24, 16, 1, 16, 0, 1, 2, 0), // 16 24 words per offset fetch
-    DD_VARIANT(DD_F32, 1, 2, 8, 16, 1, 16, 0, 1, 2, 0),  // 17
-    DD_VARIANT(DD_F32, 1, 1, 8, 16, 1, 16, 0, 1, 2, 0),  // 18
-    DD_VARIANT(DD_F32, 1, 1, 8, 4, 4, 8, 0, 1, 2, 0),    // 19
-    DD_VARIANT(DD_F32, 1, 1, 8, 1, 16, 4, 0, 1, 4, 0),   // 20 one DM per block: always fits
-    DD_VARIANT(DD_F32, 1, 2, 8, 16, 1, 16, 0, 1, 4, 1),  // 21 32-bit offsets (A/B only)
+    DD_VARIANT(DD_U16, 2, 1, 8, 16, 1, 16, 0, 1, 4, 0),  // 6  LDS.64, 16 words per offset fetch
+    DD_VARIANT(DD_U16, 1, 1, 8, 16, 1, 16, 0, 1, 4, 0),  // 7
+    DD_VARIANT(DD_U16, 1, 1, 8, 4, 4, 16, 0, 1, 4, 0),   // 8
+    DD_VARIANT(DD_U16, 1, 1, 8, 4, 4, 8, 0, 1, 4, 0),    // 9
+    DD_VARIANT(DD_U16, 1, 1, 8, 1, 16, 4, 0, 1, 4, 0),   // 10 one DM per block: always fits
+    DD_VARIANT(DD_F32, 1, 2, 24, 16, 1, 16, 0, 1, 2, 0), // 11 24 words per offset fetch
+    DD_VARIANT(DD_F32, 1, 2, 8, 16, 1, 16, 0, 1, 2, 0),  // 12
+    DD_VARIANT(DD_F32, 1, 1, 8, 16, 1, 16, 0, 1, 2, 0),  // 13
+    DD_VARIANT(DD_F32, 1, 1, 8, 4, 4, 8, 0, 1, 2, 0),    // 14
+    DD_VARIANT(DD_F32, 1, 1, 8, 1, 16, 4, 0, 1, 4, 0),   // 15 one DM per block: always fits
+#ifdef DD_TUNING
+    DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 2, 1, 4, 1),   // r01b shape: accumulators in registers
+    DD_VARIANT(DD_U8, 1, 1, 8, 16, 1, 16, 0, 1, 4, 1),   // r01 first shape
+    DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 1, 1, 4, 1),   // W on fma instead of O
+    DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 0, 1, 4, 1),   // all adds on alu
+    DD_VARIANT(DD_U16, 1, 2, 8, 16, 1, 16, 0, 1, 4, 1),  // r01b shape: 2 DMs x 8 words
+    DD_VARIANT(DD_F32, 1, 2, 8, 16, 1, 16, 0, 1, 4, 1),  // 32-bit offsets
+#endif
 };
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 

@@ -2,7 +2,6 @@
 element on the same seeded inputs.  Integer inputs: bit-exact.  float32: |gpu - oracle| <=
 1e-4 * sum_c |in| per output (BASELINE.json north_star), and bit-exact on integer-valued
 floats (every partial sum < 2^24, so any summation order gives the same float)."""
-import os
 
 import numpy as np
 import pytest
@@ -273,18 +272,18 @@ def test_repeat_execute_streams_and_host_path(B, oracle):
 
 @pytest.mark.parametrize("dtype", [np.uint8, np.uint16, np.float32])
 @pytest.mark.parametrize("case", CASES)
-def test_host_path_pipelined_chunks_match_oracle(B, oracle, dtype, case, monkeypatch):
+def test_host_path_pipelined_chunks_match_oracle(B, oracle, dtype, case):
     """dd_execute_host cuts the output into time chunks (input range = chunk + max_shift halo,
     strided 2-D copies on copy streams); 3 chunks forced here, pinned and pageable buffers,
     sentinel-filled output, ragged sizes, every dtype."""
     import torch
-    monkeypatch.setenv("DD_HOST_CHUNKS", "3")
     nchans, nsamps, ndm, step, f_high, band, tsamp = case
     rng = np.random.default_rng([nchans, nsamps, ndm, 5])
     x = _rand_input(rng, dtype, nchans, nsamps)
     dms = np.arange(ndm) * step
     plan = B.Plan(nchans, nsamps, f_high, -band / nchans, tsamp, dms,
                   {np.uint8: B.DD_U8, np.uint16: B.DD_U16, np.float32: B.DD_F32}[dtype])
+    plan.set_host_chunks(3)
     try:
         xt = torch.from_numpy(x.view(np.int16) if dtype == np.uint16 else x)
         odt = torch.float32 if dtype == np.float32 else torch.int32
@@ -367,7 +366,7 @@ U4_CASES = CASES + [(520, 3000, 9, 2.0, 1500.0, 300.0, 64e-6)]  # > 256 channels
 
 
 @pytest.mark.parametrize("case", U4_CASES)
-def test_u4_packed_input_matches_oracle(B, oracle, case, monkeypatch):
+def test_u4_packed_input_matches_oracle(B, oracle, case):
     """Two samples per byte, low nibble first (reading R14): device path, host path (3 chunks,
     odd chunk lengths) and a byte-misaligned device pointer, bit-exact against oracle.dedisperse_u4."""
     import torch
@@ -388,7 +387,7 @@ def test_u4_packed_input_matches_oracle(B, oracle, case, monkeypatch):
             plan.execute(view, d_out)
             torch.cuda.synchronize()
             assert np.array_equal(d_out.cpu().numpy().view(np.uint32), ref)
-        monkeypatch.setenv("DD_HOST_CHUNKS", "3")
+        plan.set_host_chunks(3)
         h_out = torch.full((plan.ndm, plan.out_len), -7, dtype=torch.int32).pin_memory()
         plan.execute_host(torch.from_numpy(xp).pin_memory(), h_out)
         assert np.array_equal(h_out.numpy().view(np.uint32), ref)
@@ -397,7 +396,7 @@ def test_u4_packed_input_matches_oracle(B, oracle, case, monkeypatch):
 
 
 @pytest.mark.parametrize("shape", [(256, 4096), (130, 5002), (38, 1000), (2, 300), (600, 3000)])
-def test_u4_time_major_matches_oracle(B, oracle, shape, monkeypatch):
+def test_u4_time_major_matches_oracle(B, oracle, shape):
     """Packed 4-bit delivered time-major ([nsamps][nchans/2], even channel in the low nibble,
     reading R16) through dd_execute_tm and the chunked dd_execute_host_tm."""
     import torch
@@ -414,7 +413,7 @@ def test_u4_time_major_matches_oracle(B, oracle, shape, monkeypatch):
         plan.execute_tm(torch.from_numpy(xp_tm).cuda(), d_out)
         torch.cuda.synchronize()
         assert np.array_equal(d_out.cpu().numpy().view(np.uint32), ref)
-        monkeypatch.setenv("DD_HOST_CHUNKS", "3")
+        plan.set_host_chunks(3)
         h_out = torch.full((plan.ndm, plan.out_len), -7, dtype=torch.int32).pin_memory()
         plan.execute_host_tm(torch.from_numpy(xp_tm).pin_memory(), h_out)
         assert np.array_equal(h_out.numpy().view(np.uint32), ref)
@@ -683,11 +682,8 @@ def test_fuzz_random_plans_all_rungs_bit_exact(B, oracle, seed):
             plan.execute(d_in, d_out)
             torch.cuda.synchronize()
             h_out = torch.full((ndm, out_len), -7, dtype=odt)
-            os.environ["DD_HOST_CHUNKS"] = str(int(rng.integers(1, 6)))
-            try:
-                plan.execute_host(d_in.cpu(), h_out)
-            finally:
-                os.environ.pop("DD_HOST_CHUNKS", None)
+            plan.set_host_chunks(int(rng.integers(0, 6)))
+            plan.execute_host(d_in.cpu(), h_out)
             for got in (d_out.cpu().numpy(), h_out.numpy()):
                 same = (np.array_equal(got.astype(np.float64), ref) if dt == np.float32
                         else np.array_equal(got.view(np.uint32), ref))
