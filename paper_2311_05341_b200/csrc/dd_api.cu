@@ -47,8 +47,6 @@ size_t sample_bytes(int dtype, int64_t n)
     if (dtype == DD_U4) return static_cast<size_t>(n / 2);
     return static_cast<size_t>(n) * (dtype == DD_U8 ? 1 : (dtype == DD_U16 ? 2 : 4));
 }
-// the kernel family a dtype runs through (4-bit rows are widened to 8-bit lanes by the pre-pass)
-int kernel_mode(int dtype) { return dtype == DD_U4 ? DD_U8 : dtype; }
 
 void free_device(dd_plan *p)
 {
@@ -164,7 +162,7 @@ int dd_plan_create(dd_plan **out, int nchans, int64_t nsamps, double f_high_MHz,
 #endif
         for (int v = 0; v < dd::num_variants() && !found; ++v) {
             const dd::KernelShape &sh = dd::variant_shape(v);
-            if (sh.mode != kernel_mode(in_dtype)) continue;
+            if (sh.mode != in_dtype) continue;
             if (forced >= 0 ? v != forced : sh.tune != 0) continue;
             found = dd::build_tiling(sh, v, p->table.data(), ndm, nchans, p->out_len, p->max_shift,
                                      smem_limit, &p->til);
@@ -239,7 +237,7 @@ BlockGeom geom_for(const dd_plan *plan, int64_t out_len, int64_t nsamps)
     const int NL = t.shape.lanes();
     g.L = ((out_len + NL - 1) / NL + 15) / 16 * 16;
     g.ntj = static_cast<int>((g.L + t.shape.D_J() - 1) / t.shape.D_J());
-    g.Lw = (static_cast<int64_t>(g.ntj) * t.shape.D_J() + plan->max_shift + 4 + 3) / 4 * 4;
+    g.Lw = (static_cast<int64_t>(g.ntj) * t.shape.D_J() + plan->max_shift + 4 + 7) / 8 * 8;
     return g;
 }
 
@@ -258,7 +256,8 @@ int launch_prepass(const dd_plan *plan, const BlockGeom &g, const void *d_in, in
     ip.nrows = t.nch_pad;
     ip.j_begin = 0;
     ip.j_end = g.Lw;
-    ip.nchunk = static_cast<int>((g.Lw + 1023) / 1024);
+    const int spt = plan->in_dtype == DD_U4 ? 8 : 4;  // superwords per pre-pass thread
+    ip.nchunk = static_cast<int>((g.Lw + spt * 256 - 1) / (spt * 256));
     return (time_major ? dd::launch_interleave_tm(plan->in_dtype, t.shape.VW, ip, st)
                        : dd::launch_interleave(plan->in_dtype, t.shape.VW, ip, st)) != 0
                ? DD_ERR_CUDA

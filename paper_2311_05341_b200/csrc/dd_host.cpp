@@ -76,7 +76,7 @@ bool build_tiling(const KernelShape &shape, int variant, const int32_t *table, i
     t->ndb = (ndm + D_DM - 1) / D_DM;
     t->nch_pad = static_cast<int>(round_up(nchans, CH));
     t->nk = t->nch_pad / CH;
-    t->Lw = round_up(static_cast<int64_t>(t->ntj) * D_J + max_shift + 4, 4);
+    t->Lw = round_up(static_cast<int64_t>(t->ntj) * D_J + max_shift + 4, 8);
 
     // Channel permutation: slot i of the first half of each stage takes channels from the
     // top of the band (short windows), the second half mirrors them from the bottom (long

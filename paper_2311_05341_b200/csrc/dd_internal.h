@@ -17,16 +17,16 @@ namespace dd {
 // superword-index offset: always aligned for LDS.32/64/128, whatever the shift (DESIGN.md
 // "Data layout").
 struct KernelShape {
-    int mode;     // DD_U8 / DD_U16 / DD_F32
+    int mode;     // DD_U8 / DD_U16 / DD_F32 / DD_U4 (eight 4-bit lanes per word)
     int VW;       // 32-bit words per superword: 1, 2, 4 (LDS.32 / LDS.64 / LDS.128)
     int RD, RJ;   // DM trials and superwords per thread
     int WD, WJ;   // consumer warps along DM and along j
     int CH;       // channels per pipeline stage (multiple of 8, <= 32)
-    int FM;       // u8: which adds run as IMAD on the fma pipe (dd_kernels.cu)
+    int FM;       // u8 / u4: which adds run as IMAD on the fma pipe (dd_kernels.cu)
     int NB;       // CTAs per SM the shared-memory ring is sized for
     int OW;       // bytes per shared-memory offset entry: 4 (byte offsets) or 2 (units of 4 bytes)
     int tune;     // 0: eligible for automatic selection; 1: DD_FORCE_VARIANT only
-    int lpw() const { return mode == DD_U8 ? 4 : (mode == DD_U16 ? 2 : 1); }
+    int lpw() const { return mode == DD_U4 ? 8 : (mode == DD_U8 ? 4 : (mode == DD_U16 ? 2 : 1)); }
     int lanes() const { return VW * lpw(); }
     int sw_bytes() const { return VW * 4; }
     int D_DM() const { return RD * WD; }
@@ -90,8 +90,8 @@ struct InterleaveParams {
     int64_t L, Lw;
     int nchans;        // rows nchans .. nrows-1 of X are zero-filled (padding channels)
     int nrows;
-    int64_t j_begin, j_end;  // superword columns [j_begin, j_end) of X to fill (multiples of 4)
-    int nchunk;  // blocks per channel row: ceil((j_end - j_begin) / (4 * 256)), a thread makes 4 superwords
+    int64_t j_begin, j_end;  // superword columns [j_begin, j_end) of X to fill (multiples of 8)
+    int nchunk;  // blocks per channel row: ceil((j_end - j_begin) / (SPT * 256)), a thread makes SPT = 4 (u4: 8) superwords
 };
 
 struct TransposeParams {

@@ -131,6 +131,130 @@ struct Acc<DD_U8, FM> {
         W = 0;
         O = 0;
     }
+    // the four lane sums held in the packed accumulators, which are then cleared
+    __device__ __forceinline__ void drain(uint32_t (&v)[4])
+    {
+        const uint32_t E = W - (O << 8);
+        v[0] = E & 0xFFFFu;
+        v[1] = O & 0xFFFFu;
+        v[2] = E >> 16;
+        v[3] = O >> 16;
+        W = 0;
+        O = 0;
+    }
+    static constexpr bool kNeedsFlush = true;
+};
+
+// Packed 4-bit samples, eight per 32-bit word (nibble n of a word = lane n).  Three levels:
+//   1. per stage (<= 16 channels; 17 * 15 = 255): W += x on the whole word (carries run across
+//      nibble lanes) and A += odd nibbles of x as four byte lanes (one LOP3 + one shift-and-add,
+//      SASS LEA.HI); the even nibbles are recovered exactly as byte lanes E = W - 16*A.
+//   2. at the end of every stage E and A are added into 16-bit lanes with the 8-bit trick
+//      (We += E, Oe += odd bytes of E; Wa += A, Oa += odd bytes of A): good for 4369 channels.
+//   3. every <= 4096 channels the eight 16-bit lanes of a word go to eight uint32 accumulators in
+//      tensor memory (lane-private scratch, as for 8-bit).
+// FM: 0 = W on the fma pipe (IMAD), the shift-and-add on the alu pipe; 1 = W as IADD3 as well;
+//     2 = shift and mask (SHF + LOP3) on the alu pipe, both adds as IMAD on the fma pipe
+template <int FM>
+struct Acc<DD_U4, FM> {
+    uint32_t W = 0, A = 0, Whi = 0;
+    uint32_t We = 0, Oe = 0, Wa = 0, Oa = 0;
+    static __device__ __forceinline__ uint32_t oddn(uint32_t x)
+    {
+        if (FM == 2) return (x >> 4) & 0x0F0F0F0Fu;
+        return (x & 0xF0F0F0F0u) >> 4;
+    }
+    static __device__ __forceinline__ void lea_add(uint32_t &a, uint32_t x)
+    {
+        asm("{ .reg .u32 t; and.b32 t, %1, 0xF0F0F0F0; shr.u32 t, t, 4; add.u32 %0, %0, t; }" : "+r"(a) : "r"(x));
+    }
+    static __device__ __forceinline__ void wide_add(uint32_t &lo, uint32_t &hi, uint32_t x, uint32_t one)
+    {
+        asm("{ .reg .u64 w; mov.b64 w, {%0, %1}; mad.wide.u32 w, %2, %3, w; mov.b64 {%0, %1}, w; }"
+            : "+r"(lo), "+r"(hi)
+            : "r"(x), "r"(one));
+    }
+    // first channel pair of a stage: overwrite the level-1 accumulators
+    __device__ __forceinline__ void set2(uint32_t x, uint32_t y, uint32_t one)
+    {
+        if (FM == 3) {  // A = even nibbles as byte lanes, (Whi:W) = exact 64-bit sum of the words
+            A = (x & 0x0F0F0F0Fu) + (y & 0x0F0F0F0Fu);
+            W = x;
+            Whi = 0u;
+            wide_add(W, Whi, y, one);
+        } else if (FM == 1) {
+            W = x + y;
+            A = oddn(x) + oddn(y);
+        } else if (FM == 2) {
+            W = y * one + x;
+            A = oddn(y) * one + oddn(x);
+        } else if (FM == 4) {
+            W = y * one + x;
+            A = oddn(x);
+            lea_add(A, y);
+        } else {
+            W = y * one + x;
+            A = oddn(x) + oddn(y);
+        }
+    }
+    __device__ __forceinline__ void add2(uint32_t x, uint32_t y, uint32_t one)
+    {
+        if (FM == 3) {
+            A = A + (x & 0x0F0F0F0Fu) + (y & 0x0F0F0F0Fu);
+            wide_add(W, Whi, x, one);
+            wide_add(W, Whi, y, one);
+        } else if (FM == 1) {
+            W = W + x + y;
+            A = A + oddn(x);
+            A = A + oddn(y);
+        } else if (FM == 2) {
+            W = x * one + W;
+            W = y * one + W;
+            A = oddn(x) * one + A;
+            A = oddn(y) * one + A;
+        } else if (FM == 4) {
+            W = x * one + W;
+            W = y * one + W;
+            lea_add(A, x);
+            lea_add(A, y);
+        } else {
+            W = x * one + W;
+            W = y * one + W;
+            A = A + oddn(x);
+            A = A + oddn(y);
+        }
+    }
+    // end of a stage: level 1 -> level 2
+    __device__ __forceinline__ void flush()
+    {
+        uint32_t E, O;
+        if (FM == 3) {
+            E = A;
+            const uint64_t w = (static_cast<uint64_t>(Whi) << 32 | W) - A;  // 16 * (odd nibbles as byte lanes), < 2^36
+            O = static_cast<uint32_t>(w >> 4);
+        } else {
+            E = W - (A << 4);
+            O = A;
+        }
+        We += E;
+        Oe += odd_bytes(E);
+        Wa += O;
+        Oa += odd_bytes(O);
+    }
+    // the eight lane sums held in level 2 (lane n = nibble n), which is then cleared
+    __device__ __forceinline__ void drain(uint32_t (&v)[8])
+    {
+        const uint32_t E2 = We - (Oe << 8), A2 = Wa - (Oa << 8);
+        v[0] = E2 & 0xFFFFu;
+        v[1] = A2 & 0xFFFFu;
+        v[2] = Oe & 0xFFFFu;
+        v[3] = Oa & 0xFFFFu;
+        v[4] = E2 >> 16;
+        v[5] = A2 >> 16;
+        v[6] = Oe >> 16;
+        v[7] = Oa >> 16;
+        We = Oe = Wa = Oa = 0u;
+    }
     static constexpr bool kNeedsFlush = true;
 };
 
@@ -197,20 +321,30 @@ struct SW<4> {
 // RJ superword loads of one channel row (stride 32 superwords) added into acc[.][.].
 template <int MODE, int VW, int RJ, int FM, int I = 0>
 struct RowPair {
+    // first: the first channel pair of a stage (4-bit: the per-stage accumulators are overwritten)
     static __device__ __forceinline__ void run(Acc<MODE, FM> (&acc)[RJ][VW], uint32_t a0, uint32_t a1,
-                                               uint32_t one)
+                                               uint32_t one, bool first)
     {
         SW<VW> x, y;
         x.template load<I * 32 * VW * 4>(a0);
         y.template load<I * 32 * VW * 4>(a1);
 #pragma unroll
-        for (int v = 0; v < VW; ++v) acc[I][v].add2(x.w[v], y.w[v], one);
-        RowPair<MODE, VW, RJ, FM, I + 1>::run(acc, a0, a1, one);
+        for (int v = 0; v < VW; ++v) {
+            if constexpr (MODE == DD_U4) {
+                if (first)
+                    acc[I][v].set2(x.w[v], y.w[v], one);
+                else
+                    acc[I][v].add2(x.w[v], y.w[v], one);
+            } else {
+                acc[I][v].add2(x.w[v], y.w[v], one);
+            }
+        }
+        RowPair<MODE, VW, RJ, FM, I + 1>::run(acc, a0, a1, one, first);
     }
 };
 template <int MODE, int VW, int RJ, int FM>
 struct RowPair<MODE, VW, RJ, FM, RJ> {
-    static __device__ __forceinline__ void run(Acc<MODE, FM> (&)[RJ][VW], uint32_t, uint32_t, uint32_t) {}
+    static __device__ __forceinline__ void run(Acc<MODE, FM> (&)[RJ][VW], uint32_t, uint32_t, uint32_t, bool) {}
 };
 
 template <int MODE, int VW, int RD, int RJ, int WD, int WJ, int CH, int FM, int NB, int OW>
@@ -220,7 +354,7 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
     constexpr int D_DM = RD * WD;
     constexpr int D_J = RJ * WJ * 32;  // superwords
     constexpr int S = VW * 4;          // bytes per superword
-    constexpr int LPW = MODE == DD_U8 ? 4 : (MODE == DD_U16 ? 2 : 1);
+    constexpr int LPW = MODE == DD_U4 ? 8 : (MODE == DD_U8 ? 4 : (MODE == DD_U16 ? 2 : 1));  // samples per word
     static_assert(CH % (16 / OW) == 0 && CH <= 32, "CH: whole LDS.128 offset loads, one producer lane per channel");
 
     extern __shared__ __align__(128) unsigned char smem[];
@@ -243,8 +377,12 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    constexpr bool TMEM = MODE == DD_U8 && FM == 4;
-    constexpr int NCOL = 4 * RD * RJ * VW;  // TMEM columns per consumer thread (4 uint32 per word)
+    constexpr bool TMEM = (MODE == DD_U8 && FM == 4) || MODE == DD_U4;
+    constexpr int NCOL = LPW * RD * RJ * VW;  // TMEM columns per consumer thread (one uint32 per lane of a word)
+    constexpr int WPC = 16 / LPW;             // words per 16-column tcgen05.ld / st
+    // channels between two flushes to the uint32 accumulators (16-bit lanes: 256 * 255, 4096 * 15 < 2^16)
+    constexpr int FLUSH_CH = MODE == DD_U4 ? 4096 : 256;
+    static_assert(MODE != DD_U4 || CH <= 16, "4-bit: a stage's byte lanes hold at most 17 channels");
     static_assert(!TMEM || (NCOL % 16 == 0 && (NCW + 3) / 4 * NCOL <= 512), "TMEM scratch layout");
     // columns this shape needs, rounded up to the power of two >= 32 that tcgen05.alloc takes
     constexpr int TNEED = (NCW + 3) / 4 * NCOL;
@@ -337,23 +475,31 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
                     for (int h = 0; h < 4; ++h) {
                         const uint32_t a0 = (o[r][h] & 0xffffu) * four + rows;
                         const uint32_t a1 = (o[r][h] >> 16) * four + rows;
-                        RowPair<MODE, VW, RJ, FM>::run(acc[r], a0, a1, one);
+                        RowPair<MODE, VW, RJ, FM>::run(acc[r], a0, a1, one, cg == 0 && h == 0);
                     }
                 } else {
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
                         const uint32_t a0 = o[r][2 * h] * one + rows;
                         const uint32_t a1 = o[r][2 * h + 1] * one + rows;
-                        RowPair<MODE, VW, RJ, FM>::run(acc[r], a0, a1, one);
+                        RowPair<MODE, VW, RJ, FM>::run(acc[r], a0, a1, one, cg == 0 && h == 0);
                     }
                 }
             }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_empty + 8u * s);
-        // u8: the packed 16-bit lanes hold at most 256 channels (256 * 255 < 2^16) between flushes
+        if constexpr (MODE == DD_U4) {  // the stage's byte lanes -> 16-bit lanes
+#pragma unroll
+            for (int r = 0; r < RD; ++r)
+#pragma unroll
+                for (int i = 0; i < RJ; ++i)
+#pragma unroll
+                    for (int v = 0; v < VW; ++v) acc[r][i][v].flush();
+        }
+        // the packed 16-bit lanes hold at most FLUSH_CH channels between flushes
         since_flush += CH;
-        if (Acc<MODE, FM>::kNeedsFlush && since_flush + CH > 256) {
+        if (Acc<MODE, FM>::kNeedsFlush && since_flush + CH > FLUSH_CH) {
             since_flush = 0;
             if constexpr (TMEM) {
                 if (k + 1 < p.nk) {  // (the last stage's sums go straight to the epilogue)
@@ -367,16 +513,12 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
                             for (int q = 0; q < 16; ++q) t[q] = 0u;
                         }
 #pragma unroll
-                        for (int q = 0; q < 4; ++q) {
-                            const int wi = ch * 4 + q;
-                            Acc<MODE, FM> &a = acc[wi / (RJ * VW)][(wi / VW) % RJ][wi % VW];
-                            const uint32_t E = a.W - (a.O << 8);
-                            t[q * 4 + 0] += E & 0xFFFFu;
-                            t[q * 4 + 1] += a.O & 0xFFFFu;
-                            t[q * 4 + 2] += E >> 16;
-                            t[q * 4 + 3] += a.O >> 16;
-                            a.W = 0;
-                            a.O = 0;
+                        for (int q = 0; q < WPC; ++q) {
+                            const int wi = ch * WPC + q;
+                            uint32_t val[LPW];
+                            acc[wi / (RJ * VW)][(wi / VW) % RJ][wi % VW].drain(val);
+#pragma unroll
+                            for (int l = 0; l < LPW; ++l) t[q * LPW + l] += val[l];
                         }
                         tmem_st16(taddr + ch * 16, t);
                     }
@@ -410,21 +552,19 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
                 for (int q = 0; q < 16; ++q) t[q] = 0u;
             }
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const int wi = ch * 4 + q;
+            for (int q = 0; q < WPC; ++q) {
+                const int wi = ch * WPC + q;
                 const int r = wi / (RJ * VW), i = (wi / VW) % RJ, v = wi % VW;
-                const Acc<MODE, FM> &a = acc[r][i][v];
-                const uint32_t E = a.W - (a.O << 8);
-                const uint32_t val[4] = {t[q * 4 + 0] + (E & 0xFFFFu), t[q * 4 + 1] + (a.O & 0xFFFFu),
-                                         t[q * 4 + 2] + (E >> 16), t[q * 4 + 3] + (a.O >> 16)};
+                uint32_t val[LPW];
+                acc[r][i][v].drain(val);
                 const int d = b * D_DM + wd * RD + r;
                 const int64_t j = j0 + (wj * RJ + i) * 32 + lane;
                 if (d < p.ndm && j < p.L) {
                     uint32_t *o = static_cast<uint32_t *>(p.out) + static_cast<size_t>(d) * p.out_pitch;
 #pragma unroll
-                    for (int l = 0; l < 4; ++l) {
-                        const int64_t tt = static_cast<int64_t>(v * 4 + l) * p.L + j;
-                        if (tt < p.out_len) o[tt] = val[l];
+                    for (int l = 0; l < LPW; ++l) {
+                        const int64_t tt = static_cast<int64_t>(v * LPW + l) * p.L + j;
+                        if (tt < p.out_len) o[tt] = t[q * LPW + l] + val[l];
                     }
                 }
             }
@@ -444,7 +584,7 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
             if (j >= p.L) continue;
 #pragma unroll
             for (int v = 0; v < VW; ++v) {
-                uint32_t val[LPW];
+                uint32_t val[LPW] = {};
                 if constexpr (MODE == DD_U8) {
                     Acc<DD_U8, FM> &a = acc[r][i][v];
                     a.flush();
@@ -456,7 +596,7 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
                     Acc<DD_U16, FM> &a = acc[r][i][v];
                     val[0] = a.W - (a.H << 16);
                     val[1] = a.H;
-                } else {
+                } else if constexpr (MODE == DD_F32) {
                     val[0] = __float_as_uint(acc[r][i][v].s);
                 }
                 uint32_t *o = static_cast<uint32_t *>(p.out) + static_cast<size_t>(d) * p.out_pitch;
@@ -490,37 +630,6 @@ __global__ void __launch_bounds__(256) interleave_kernel(const InterleaveParams 
     if (c >= p.nchans) {  // padding channel (nchans rounded up to CH): a zero row
 #pragma unroll
         for (int i = 0; i < 4 * VW; ++i) w[i] = 0u;
-    } else if (MODE == DD_U4) {
-        // packed 4-bit rows (two samples per byte, earlier sample in the low nibble) are widened
-        // to the u8 lane layout here; the main kernel is the u8 one
-        const uint8_t *row = static_cast<const uint8_t *>(p.in) + static_cast<size_t>(c) * (p.in_pitch / 2);
-        const bool aligned = (reinterpret_cast<uintptr_t>(row) & 1u) == 0;
-#pragma unroll
-        for (int v = 0; v < VW; ++v) {
-            uint32_t seg[4];
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const int64_t t = (v * 4 + k) * p.L + j;  // multiple of 4: starts on a byte
-                uint32_t h = 0;
-                if (aligned && t + 3 < p.nsamps) {
-                    h = *reinterpret_cast<const uint16_t *>(row + (t >> 1));
-                } else {
-                    if (t < p.nsamps) h = row[t >> 1];
-                    if (t + 2 < p.nsamps) h |= static_cast<uint32_t>(row[(t >> 1) + 1]) << 8;
-                    if (t + 1 >= p.nsamps) h &= 0x000Fu;       // odd valid length: drop the
-                    else if (t + 3 >= p.nsamps) h &= 0x0FFFu;  // nibbles past the end
-                }
-                seg[k] = (h & 0x000Fu) | (h & 0x00F0u) << 4 | (h & 0x0F00u) << 8 | (h & 0xF000u) << 12;
-            }
-            const uint32_t t01l = __byte_perm(seg[0], seg[1], 0x5140);
-            const uint32_t t01h = __byte_perm(seg[0], seg[1], 0x7362);
-            const uint32_t t23l = __byte_perm(seg[2], seg[3], 0x5140);
-            const uint32_t t23h = __byte_perm(seg[2], seg[3], 0x7362);
-            w[0 * VW + v] = __byte_perm(t01l, t23l, 0x5410);
-            w[1 * VW + v] = __byte_perm(t01l, t23l, 0x7632);
-            w[2 * VW + v] = __byte_perm(t01h, t23h, 0x5410);
-            w[3 * VW + v] = __byte_perm(t01h, t23h, 0x7632);
-        }
     } else if (MODE == DD_U8) {
         const uint8_t *row = static_cast<const uint8_t *>(p.in) + static_cast<size_t>(c) * p.in_pitch;
         const bool aligned = (reinterpret_cast<uintptr_t>(row) & 3u) == 0;
@@ -624,6 +733,98 @@ __global__ void __launch_bounds__(256) interleave_kernel(const InterleaveParams 
     uint4 *dst = reinterpret_cast<uint4 *>(p.X + (static_cast<size_t>(c) * p.Lw + j) * VW);
 #pragma unroll
     for (int i = 0; i < VW; ++i) dst[i] = make_uint4(w[4 * i], w[4 * i + 1], w[4 * i + 2], w[4 * i + 3]);
+}
+
+// 8 x 8 transpose of 4-bit elements: on entry nibble q of r[n] is element (n, q), on return
+// nibble n of r[q] is element (n, q).  16-bit and 8-bit block swaps with PRMT, the last level
+// with shifts and masks (32 instructions for 64 elements).
+__device__ __forceinline__ void transpose_nibbles_8x8(uint32_t (&r)[8])
+{
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const uint32_t a = r[i], b = r[i + 4];
+        r[i] = __byte_perm(a, b, 0x5410);
+        r[i + 4] = __byte_perm(a, b, 0x7632);
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        if (i & 2) continue;
+        const uint32_t a = r[i], b = r[i + 2];
+        r[i] = __byte_perm(a, b, 0x6240);
+        r[i + 2] = __byte_perm(a, b, 0x7351);
+    }
+#pragma unroll
+    for (int i = 0; i < 8; i += 2) {
+        const uint32_t a = r[i], b = r[i + 1];
+        r[i] = (a & 0x0F0F0F0Fu) | ((b << 4) & 0xF0F0F0F0u);
+        r[i + 1] = ((a >> 4) & 0x0F0F0F0Fu) | (b & 0xF0F0F0F0u);
+    }
+}
+
+// Packed 4-bit rows (two samples per byte, the earlier one in the low nibble; DESIGN.md reading
+// R14) -> superwords of VW words of EIGHT 4-bit lanes: nibble n of word v of X[c][j] is
+// in[c][(8v + n)*L + j].  One thread makes eight consecutive superwords of one channel from
+// 8*VW eight-sample segments (one 32-bit load each) and VW 8 x 8 nibble transposes.
+template <int VW>
+__global__ void __launch_bounds__(256) interleave_u4_kernel(const InterleaveParams p)
+{
+    const int c = static_cast<int>(blockIdx.x / p.nchunk);
+    const int64_t j = p.j_begin + (static_cast<int64_t>(blockIdx.x % p.nchunk) * blockDim.x + threadIdx.x) * 8;
+    if (j >= p.j_end) return;
+    uint32_t w[VW][8];  // w[v][q] = word v of superword j + q
+    if (c >= p.nchans) {
+#pragma unroll
+        for (int v = 0; v < VW; ++v)
+#pragma unroll
+            for (int q = 0; q < 8; ++q) w[v][q] = 0u;
+    } else {
+        const uint8_t *row = static_cast<const uint8_t *>(p.in) + static_cast<size_t>(c) * (p.in_pitch / 2);
+        const bool aligned = (reinterpret_cast<uintptr_t>(row) & 3u) == 0;
+        // every segment in range: issue all loads before any is used
+        const bool fast = aligned && (8 * VW - 1) * p.L + j + 7 < p.nsamps;
+        if (fast) {
+#pragma unroll
+            for (int v = 0; v < VW; ++v)
+#pragma unroll
+                for (int n = 0; n < 8; ++n)
+                    w[v][n] = *reinterpret_cast<const uint32_t *>(row + (((v * 8 + n) * p.L + j) >> 1));
+        } else {
+#pragma unroll
+            for (int v = 0; v < VW; ++v)
+#pragma unroll
+                for (int n = 0; n < 8; ++n) {
+                    const int64_t t = (v * 8 + n) * p.L + j;  // multiple of 8: starts on a byte
+                    uint32_t x = 0u;
+                    if (aligned && t + 7 < p.nsamps) {
+                        x = *reinterpret_cast<const uint32_t *>(row + (t >> 1));
+                    } else {
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) {
+                            uint32_t byte = 0u;
+                            if (t + 2 * k < p.nsamps) byte = row[(t >> 1) + k];
+                            if (t + 2 * k + 1 >= p.nsamps) byte &= 0x0Fu;  // odd valid length: drop the nibble past the end
+                            x |= byte << (8 * k);
+                        }
+                    }
+                    w[v][n] = x;
+                }
+        }
+#pragma unroll
+        for (int v = 0; v < VW; ++v) transpose_nibbles_8x8(w[v]);
+    }
+    uint32_t *dst = p.X + (static_cast<size_t>(c) * p.Lw + j) * VW;
+    if constexpr (VW == 1) {
+        *reinterpret_cast<uint4 *>(dst) = make_uint4(w[0][0], w[0][1], w[0][2], w[0][3]);
+        *reinterpret_cast<uint4 *>(dst + 4) = make_uint4(w[0][4], w[0][5], w[0][6], w[0][7]);
+    } else if constexpr (VW == 2) {
+#pragma unroll
+        for (int q = 0; q < 8; q += 2)
+            *reinterpret_cast<uint4 *>(dst + q * 2) = make_uint4(w[0][q], w[1][q], w[0][q + 1], w[1][q + 1]);
+    } else {
+#pragma unroll
+        for (int q = 0; q < 8; ++q)
+            *reinterpret_cast<uint4 *>(dst + q * 4) = make_uint4(w[0][q], w[1][q], w[2][q], w[3][q]);
+    }
 }
 
 // ------------------------------------------------------------------ transpose pre-step
@@ -802,14 +1003,15 @@ __global__ void __launch_bounds__(256) interleave_tm_kernel(const InterleavePara
 }
 
 // The same for packed 4-bit time-major input [nsamps][nchans/2 bytes] (reading R16: the even
-// channel of a byte in the low nibble): a tile is 128 bytes = 256 channels; phase 2 splits each
-// word into its low-nibble and high-nibble bytes (even / odd channels) before the 4 x 4 byte
-// transposes, so a thread stores the u8-lane superwords of eight channels.
+// channel of a byte in the low nibble), into the eight-lanes-per-word layout of
+// interleave_u4_kernel: a tile is 128 bytes = 256 channels x TJ superword columns; in phase 2 a
+// thread takes the words of one column and eight channels from the 8*VW lane rows, transposes
+// 8 x 8 nibbles per superword word (lane <-> channel) and stores the superwords of its channels.
 template <int VW>
 __global__ void __launch_bounds__(256) interleave_tm_u4_kernel(const InterleaveParams p)
 {
-    constexpr int NL = VW * 4;
-    constexpr int TJ = NL > 8 ? 16 : 32;
+    constexpr int NL = VW * 8;
+    constexpr int TJ = 256 / NL;
     __shared__ uint32_t tile[NL * TJ][33];
     const uint8_t *in = static_cast<const uint8_t *>(p.in);
     const int64_t pb = p.in_pitch / 2;  // bytes per time row
@@ -848,26 +1050,12 @@ __global__ void __launch_bounds__(256) interleave_tm_u4_kernel(const InterleaveP
     for (int q = threadIdx.x; q < 32 * TJ; q += 256) {
         const int j = q % TJ, cw = q / TJ;
         if (j0 + j >= p.Lw) continue;
-        uint32_t o[8][VW];  // o[2*b + parity][v]: word v of channel c0 + cw*8 + 2*b + parity
+        uint32_t o[VW][8];  // o[v][k]: word v of channel c0 + cw*8 + k
 #pragma unroll
         for (int v = 0; v < VW; ++v) {
-            uint32_t lo[4], hi[4];
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const uint32_t w = tile[(4 * v + i) * TJ + j][cw];
-                lo[i] = w & 0x0F0F0F0Fu;
-                hi[i] = (w >> 4) & 0x0F0F0F0Fu;
-            }
-#pragma unroll
-            for (int par = 0; par < 2; ++par) {
-                const uint32_t *x = par ? hi : lo;
-                const uint32_t a = __byte_perm(x[0], x[1], 0x5140), b2 = __byte_perm(x[0], x[1], 0x7362);
-                const uint32_t c2 = __byte_perm(x[2], x[3], 0x5140), d2 = __byte_perm(x[2], x[3], 0x7362);
-                o[0 + par][v] = __byte_perm(a, c2, 0x5410);
-                o[2 + par][v] = __byte_perm(a, c2, 0x7632);
-                o[4 + par][v] = __byte_perm(b2, d2, 0x5410);
-                o[6 + par][v] = __byte_perm(b2, d2, 0x7632);
-            }
+            for (int n = 0; n < 8; ++n) o[v][n] = tile[(8 * v + n) * TJ + j][cw];  // nibble k = channel k at lane 8v + n
+            transpose_nibbles_8x8(o[v]);
         }
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
@@ -875,11 +1063,11 @@ __global__ void __launch_bounds__(256) interleave_tm_u4_kernel(const InterleaveP
             if (c >= p.nrows) continue;
             uint32_t *dst = p.X + (static_cast<size_t>(c) * p.Lw + j0 + j) * VW;
             if constexpr (VW == 1)
-                dst[0] = o[k][0];
+                dst[0] = o[0][k];
             else if constexpr (VW == 2)
-                *reinterpret_cast<uint2 *>(dst) = make_uint2(o[k][0], o[k][1]);
+                *reinterpret_cast<uint2 *>(dst) = make_uint2(o[0][k], o[1][k]);
             else
-                *reinterpret_cast<uint4 *>(dst) = make_uint4(o[k][0], o[k][1], o[k][2], o[k][3]);
+                *reinterpret_cast<uint4 *>(dst) = make_uint4(o[0][k], o[1][k], o[2][k], o[3][k]);
         }
     }
 }
@@ -1070,7 +1258,25 @@ const Variant kVariants[] = {
     DD_VARIANT(DD_F32, 1, 1, 8, 16, 1, 16, 0, 1, 2, 0),  // 13
     DD_VARIANT(DD_F32, 1, 1, 8, 4, 4, 8, 0, 1, 2, 0),    // 14
     DD_VARIANT(DD_F32, 1, 1, 8, 1, 16, 4, 0, 1, 4, 0),   // 15 one DM per block: always fits
+    // u4: eight 4-bit lanes per word, LDS.64 superwords of 16 samples, 12 DM warps x 8 superwords,
+    // odd nibbles by LOP3 + LEA.HI on the alu pipe, the whole-word add on the fma pipe (FM = 4)
+    DD_VARIANT(DD_U4, 2, 1, 8, 12, 1, 16, 4, 1, 4, 0),   // 16
+    DD_VARIANT(DD_U4, 2, 1, 8, 12, 1, 8, 4, 1, 4, 0),    // 17
+    DD_VARIANT(DD_U4, 2, 1, 8, 6, 2, 8, 4, 1, 4, 0),     // 18
+    DD_VARIANT(DD_U4, 2, 1, 8, 3, 4, 4, 4, 1, 4, 0),     // 19
+    DD_VARIANT(DD_U4, 2, 1, 4, 3, 4, 4, 4, 1, 4, 0),     // 20
+    DD_VARIANT(DD_U4, 2, 1, 4, 1, 12, 4, 4, 1, 4, 0),    // 21 one DM per block: always fits
 #ifdef DD_TUNING
+    DD_VARIANT(DD_U4, 2, 1, 8, 12, 1, 16, 0, 1, 4, 1),   // 22 compiler's choice of shift-and-add
+    DD_VARIANT(DD_U4, 2, 1, 8, 12, 1, 16, 2, 1, 4, 1),   // 23 SHF + LOP3, both adds on fma
+    DD_VARIANT(DD_U4, 2, 1, 6, 12, 1, 16, 4, 1, 4, 1),   // 24 6 superwords
+    DD_VARIANT(DD_U4, 4, 1, 4, 12, 1, 16, 4, 1, 4, 1),   // 25 LDS.128 x 4
+    DD_VARIANT(DD_U4, 4, 1, 3, 12, 1, 16, 4, 1, 4, 1),   // 26 LDS.128 x 3
+    DD_VARIANT(DD_U4, 2, 1, 8, 12, 1, 16, 3, 1, 4, 1),   // 27 IMAD.WIDE 64-bit whole-word sum
+    DD_VARIANT(DD_U4, 2, 1, 8, 12, 1, 16, 1, 1, 4, 1),   // 28 W as IADD3
+    DD_VARIANT(DD_U4, 2, 1, 8, 8, 1, 16, 4, 1, 4, 1),    // 29 8 DM warps
+    DD_VARIANT(DD_U4, 2, 1, 4, 12, 2, 16, 4, 1, 4, 1),   // 30 24 warps x 4 superwords
+    DD_VARIANT(DD_U4, 2, 1, 8, 11, 1, 16, 4, 1, 4, 1),   // 31 11 DM warps (12 warps in all: 168 registers)
     DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 2, 1, 4, 1),   // r01b shape: accumulators in registers
     DD_VARIANT(DD_U8, 1, 1, 8, 16, 1, 16, 0, 1, 4, 1),   // r01 first shape
     DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 1, 1, 4, 1),   // W on fma instead of O
@@ -1104,7 +1310,7 @@ template <int VW>
 static void launch_interleave_vw(int mode, const InterleaveParams &p, unsigned grid, cudaStream_t st)
 {
     if (mode == DD_U4)
-        interleave_kernel<DD_U4, VW><<<grid, 256, 0, st>>>(p);
+        interleave_u4_kernel<VW><<<grid, 256, 0, st>>>(p);
     else if (mode == DD_U8)
         interleave_kernel<DD_U8, VW><<<grid, 256, 0, st>>>(p);
     else if (mode == DD_U16)
@@ -1192,7 +1398,7 @@ int launch_interleave_tm(int mode, int VW, const InterleaveParams &p, void *stre
 {
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if (mode == DD_U4) {
-        const int TJ4 = VW * 4 > 8 ? 16 : 32;
+        const int TJ4 = 256 / (VW * 8);
         const unsigned g4 = static_cast<unsigned>((p.Lw + TJ4 - 1) / TJ4 * ((p.nrows + 255) / 256));
         if (VW == 1)
             interleave_tm_u4_kernel<1><<<g4, 256, 0, st>>>(p);
