@@ -219,7 +219,7 @@ def _dtype_name(cfg):
     return {W.U8: "u8 in, packed u16/u32 integer accumulate, u32 out",
             W.U16: "u16 in, u32 integer accumulate, u32 out",
             W.F32: "f32",
-            W.U4: "u4 in (widened to u8 lanes by the pre-pass), packed u16/u32 integer accumulate, u32 out"}[cfg.in_dtype]
+            W.U4: "u4 in (eight 4-bit lanes per word on chip), packed u8/u16/u32 integer accumulate, u32 out"}[cfg.in_dtype]
 
 
 class _OracleFacts:
@@ -463,7 +463,7 @@ def run_ours(args):
     smem_peak_derived = N_SM * SMEM_BYTES_PER_SM_CLK * sm_max_mhz * 1e6 / 1e9
     int_peak_derived = N_SM * INT_LANES_PER_SM_CLK * sm_max_mhz * 1e6
     in_b = W.ELEM_BYTES[cfg.in_dtype]
-    smem_b = 1 if cfg.in_dtype == W.U4 else in_b        # 4-bit samples travel as bytes on chip
+    smem_b = in_b                                       # bytes a sample occupies in shared memory (4-bit: 0.5)
     smem_alg_bytes = adds * smem_b                      # one sample read from shared memory per add
     hbm_alg_bytes = int(cfg.nchans * cfg.nsamps * in_b) + plan.ndm * plan.out_len * 4
     traffic = None
@@ -491,7 +491,22 @@ def run_ours(args):
                     "peak_kind": "measured (dd_probe): %.1f IADD3 lanes/clk/SM x %d SMs x %.0f MHz; derived %.2f Tadd/s"
                                  % (probed["IADD3"], n_sm, probed["SM_CLOCK_MHZ"], int_peak_derived / 1e12),
                     "note": "sample-adds against one-add-per-lane integer peak (BASELINE.json's metric); "
-                            "a packed add performs 4 (u8) / 2 (u16) sample-adds, so frac may exceed 1"}
+                            "a packed add performs 8 (u4) / 4 (u8) / 2 (u16) sample-adds, so frac may exceed 1"}
+    if cfg.in_dtype == W.U4:
+        # The 4-bit kernel is bound by the alu pipe, not by shared memory (ncu:
+        # alu 83 % busy, shared-memory wavefronts 76 %): per 32-bit word (8 sample-adds) the odd
+        # nibbles cost one LOP3 and one LEA.HI there, which no formulation found avoids.  The
+        # shared-memory view is kept beside it.
+        alu_ops = adds * 2.0 / 8.0
+        roofline_smem = roofline
+        roofline = {"bound": "alu", "kernel": "dedisperse_kernel", "achieved": alu_ops / main_s / 1e12,
+                    "peak": int_peak / 1e12, "unit": "T lane-instructions/s",
+                    "frac": alu_ops / main_s / int_peak, "traffic": traffic,
+                    "traffic_note": roofline_smem["traffic_note"],
+                    "peak_kind": "measured (dd_probe): %.1f alu-pipe lanes/clk/SM x %d SMs x %.0f MHz"
+                                 % (probed["IADD3"], n_sm, probed["SM_CLOCK_MHZ"]),
+                    "algorithmic_alu_instructions_per_add": 0.25, "adds_per_launch": adds,
+                    "kernel_ms": main_s * 1e3, "share_of_step": share, "smem_view": roofline_smem}
     roofline_hbm = {"bound": "hbm", "achieved": hbm_alg_bytes / (ms_step * 1e-3) / 1e9, "peak": hbm_gbs,
                     "unit": "GB/s", "frac": hbm_alg_bytes / (ms_step * 1e-3) / 1e9 / hbm_gbs,
                     "peak_kind": peak_kind + " copy bandwidth",

@@ -184,7 +184,8 @@ enum {
     DD_INFO_STAGE_BYTES = 8,   /* bytes the main kernel stages global->shared per launch */
     DD_INFO_LAUNCHES = 9,      /* kernels dd_execute launches */
     DD_INFO_CH = 10,           /* channels per pipeline stage */
-    DD_INFO_NSTAGE = 11        /* pipeline stages */
+    DD_INFO_NSTAGE = 11,       /* pipeline stages */
+    DD_INFO_PANEL = 12         /* DM blocks per rasterisation panel of the main kernel's grid */
 };
 int64_t dd_plan_info(const dd_plan *plan, int what);
 

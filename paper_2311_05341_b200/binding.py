@@ -24,7 +24,7 @@ DD_ERR_UNSUPPORTED_DEVICE = -6
 DD_ERR_UNSUPPORTED_PLAN = -7
 
 INFO = {"D_DM": 0, "D_J": 1, "LANES": 2, "L": 3, "SMEM_BYTES": 4, "GRID": 5, "THREADS": 6,
-        "WORKSPACE_BYTES": 7, "STAGE_BYTES": 8, "LAUNCHES": 9, "CH": 10, "NSTAGE": 11}
+        "WORKSPACE_BYTES": 7, "STAGE_BYTES": 8, "LAUNCHES": 9, "CH": 10, "NSTAGE": 11, "PANEL": 12}
 
 # every symbol include/dd.h declares (tests check the .so exports all of them)
 SYMBOLS = ("dd_shift_table_build", "dd_plan_create", "dd_plan_shift_table", "dd_execute",

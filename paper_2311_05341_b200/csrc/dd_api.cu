@@ -26,6 +26,7 @@ struct dd_plan {
     void *d_in_own = nullptr, *d_out_own = nullptr;
     static constexpr int kHostChunks = 8;
     bool host_made = false;
+    int panel_override = 0;  // tuning builds: DD_PANEL
     int host_chunks = 0;  // dd_plan_set_host_chunks: 0 = default tapered schedule, n = n equal chunks
     cudaStream_t st_h2d = nullptr, st_d2h = nullptr, st_pre = nullptr, st_main2 = nullptr;
     cudaEvent_t ev_in[kHostChunks + 1] = {}, ev_done[kHostChunks + 1] = {}, ev_pre[kHostChunks + 1] = {};
@@ -157,6 +158,7 @@ int dd_plan_create(dd_plan **out, int nchans, int64_t nsamps, double f_high_MHz,
 #ifdef DD_TUNING
         const char *force = std::getenv("DD_FORCE_VARIANT");  // tuning builds only (build.py --tuning)
         const int forced = force ? std::atoi(force) : -1;
+        if (const char *pe = std::getenv("DD_PANEL")) p->panel_override = std::atoi(pe);
 #else
         const int forced = -1;
 #endif
@@ -165,7 +167,7 @@ int dd_plan_create(dd_plan **out, int nchans, int64_t nsamps, double f_high_MHz,
             if (sh.mode != in_dtype) continue;
             if (forced >= 0 ? v != forced : sh.tune != 0) continue;
             found = dd::build_tiling(sh, v, p->table.data(), ndm, nchans, p->out_len, p->max_shift,
-                                     smem_limit, &p->til);
+                                     smem_limit, prop.multiProcessorCount, &p->til);
         }
         if (!found) {
             p->device = -1;
@@ -281,6 +283,7 @@ int launch_main(const dd_plan *plan, const BlockGeom &g, const uint32_t *X, void
     kp.nch_pad = t.nch_pad;
     kp.nk = t.nk;
     kp.ndb = t.ndb;
+    kp.panel = plan->panel_override > 0 ? (plan->panel_override < t.ndb ? plan->panel_override : t.ndb) : t.panel;
     kp.ntj = g.ntj;
     kp.jt_begin = 0;
     kp.rows_bytes = t.rows_bytes;
@@ -637,6 +640,7 @@ int64_t dd_plan_info(const dd_plan *plan, int what)
     case DD_INFO_LAUNCHES: return 2;
     case DD_INFO_CH: return t.shape.CH;
     case DD_INFO_NSTAGE: return t.nstage;
+    case DD_INFO_PANEL: return t.panel;
     default: return -1;
     }
 }

@@ -64,7 +64,7 @@ int build_shift_table(int nchans, double f_high, double chan_bw, double tsamp,
 // inside the stage buffer.  Windows are packed back to back in a stage.
 bool build_tiling(const KernelShape &shape, int variant, const int32_t *table, int ndm,
                   int nchans, int64_t out_len, int32_t max_shift, int64_t smem_limit,
-                  Tiling *t)
+                  int num_sms, Tiling *t)
 {
     const int D_DM = shape.D_DM(), D_J = shape.D_J(), CH = shape.CH;
     const int S = shape.sw_bytes();  // bytes per superword
@@ -140,6 +140,23 @@ bool build_tiling(const KernelShape &shape, int variant, const int32_t *table, i
     if (nstage < 2) return false;
     t->nstage = nstage;
     t->smem_bytes = barrier_bytes + nstage * stage_bytes;
+    // Rasterisation panel (dd_kernels.cu): a wave of num_sms CTAs covering nb DM blocks x
+    // num_sms/nb j tiles touches about nb * span + (num_sms/nb) * tile bytes of X, where tile =
+    // one j tile of every channel and span = what one more DM block adds to the staged windows
+    // (the shift difference across the block, summed over channels).  Minimal at
+    // nb = sqrt(num_sms * tile / span); panels are made equal.
+    {
+        double span = 0.0;
+        for (int c = 0; c < nchans; ++c)
+            span += static_cast<double>(table[static_cast<size_t>(ndm - 1) * nchans + c] - table[c]);
+        span = span * S / t->ndb;
+        const double tile = static_cast<double>(t->nch_pad) * D_J * S;
+        double nb = span > 0.0 ? std::sqrt(static_cast<double>(num_sms) * tile / span) : t->ndb;
+        if (nb < 1.0) nb = 1.0;
+        if (nb > t->ndb) nb = t->ndb;
+        const int npanel = std::max(1, static_cast<int>(std::lround(t->ndb / nb)));
+        t->panel = (t->ndb + npanel - 1) / npanel;
+    }
     t->stage_bytes_total =
         (per_jtile_bytes + static_cast<int64_t>(t->ndb) * t->nk * ofs_stage_bytes) * t->ntj;
 

@@ -41,6 +41,7 @@ struct Tiling {
     int64_t Lw = 0;            // superwords per row of the interleaved workspace X
     int nch_pad = 0;           // nchans rounded up to CH (padding rows of X stay zero)
     int ndb = 0, ntj = 0, nk = 0;  // DM blocks, j tiles, channel stages
+    int panel = 1;             // DM blocks per rasterisation panel of the main kernel's grid
     int rows_bytes = 0;        // bytes of channel windows in one stage buffer (multiple of 16)
     int nstage = 0;
     int64_t smem_bytes = 0;
@@ -62,7 +63,7 @@ int build_shift_table(int nchans, double f_high, double chan_bw, double tsamp,
 // Fill `t` for the given shape; returns false when even NSTAGE = 2 does not fit `smem_limit`.
 bool build_tiling(const KernelShape &shape, int variant, const int32_t *table, int ndm,
                   int nchans, int64_t out_len, int32_t max_shift, int64_t smem_limit,
-                  Tiling *t);
+                  int num_sms, Tiling *t);
 
 // ---- device side -------------------------------------------------------------------------
 struct KernelParams {
@@ -75,6 +76,7 @@ struct KernelParams {
     int64_t Lw;        // superwords per row of X
     int64_t L;
     int ndm, nch_pad, nk, ndb, ntj;
+    int panel;         // DM blocks per rasterisation panel (1 .. ndb)
     int jt_begin;      // first j tile of this launch (the grid covers a range of tiles)
     int rows_bytes;    // channel windows of one stage; the stage's offset table follows
     int nstage;

@@ -347,6 +347,21 @@ struct RowPair<MODE, VW, RJ, FM, RJ> {
     static __device__ __forceinline__ void run(Acc<MODE, FM> (&)[RJ][VW], uint32_t, uint32_t, uint32_t, bool) {}
 };
 
+// Rasterisation of the main kernel's grid: DM blocks are grouped in panels of p.panel; inside a
+// panel the DM block runs fastest, then the j tile.  The CTAs resident at one time (one wave)
+// then cover ~panel DM blocks x (SMs / panel) j tiles, the shape that minimises the input
+// footprint of a wave -- every wave streams its footprint from HBM once (DESIGN.md "DRAM
+// traffic").  Returns the DM block and the j tile of CTA `bid`.
+__device__ __forceinline__ void tile_of_cta(const KernelParams &p, int bid, int &b, int &jt)
+{
+    const int per_panel = p.panel * p.ntj;
+    const int pn = bid / per_panel;
+    const int rem = bid - pn * per_panel;
+    const int nb = min(p.panel, p.ndb - pn * p.panel);
+    b = pn * p.panel + rem % nb;
+    jt = rem / nb + p.jt_begin;
+}
+
 template <int MODE, int VW, int RD, int RJ, int WD, int WJ, int CH, int FM, int NB, int OW>
 __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(const KernelParams p)
 {
@@ -365,9 +380,6 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
     unsigned char *stage0 = smem + 1024;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int b = blockIdx.x % p.ndb;  // DM block fastest: co-resident blocks share input
-    const int jt = blockIdx.x / p.ndb + p.jt_begin;
-    const int64_t j0 = static_cast<int64_t>(jt) * D_J;
     const int nstage = p.nstage;
 
     if (threadIdx.x == 0) {
@@ -392,14 +404,13 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     __syncthreads();
-    uint32_t tmem = 0;
-    if (TMEM) {
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem) : "r"(bar_full + 960u) : "memory");
-    }
+    if (TMEM) asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 
     if (warp == NCW) {
         // ===================== producer warp: lane l stages slot l of each stage
+        int b, jt;
+        tile_of_cta(p, blockIdx.x, b, jt);
+        const int64_t j0 = static_cast<int64_t>(jt) * D_J;
         const int4 *blk = reinterpret_cast<const int4 *>(p.blk) + static_cast<size_t>(b) * p.nch_pad;
         const unsigned char *ofs_blk =
             static_cast<const unsigned char *>(p.ofs) + static_cast<size_t>(b) * p.nk * (D_DM * CH * OW);
@@ -446,7 +457,13 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
     // [(warp / 4) * NCOL, +NCOL) of lane quarter warp % 4 (the hardware's rule: warp w of a CTA
     // reaches lanes 32 * (w % 4) .. +31); column ((r*RJ + i)*VW + v)*4 + l.  Touched only at a
     // flush (every 256 channels) and at the end, 16 columns per instruction.
-    const uint32_t taddr = tmem + (static_cast<uint32_t>((warp & 3) * 32) << 16) + static_cast<uint32_t>((warp >> 2) * NCOL);
+    // (the address is re-read from shared memory at each of its rare uses: the hot loop is at the
+    // register limit)
+    auto tmem_addr = [&]() {
+        uint32_t base;
+        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(base) : "r"(bar_full + 960u) : "memory");
+        return base + (static_cast<uint32_t>((warp & 3) * 32) << 16) + static_cast<uint32_t>((warp >> 2) * NCOL);
+    };
     bool parked = false;  // TMEM holds valid partial sums
     int s = 0;
     int since_flush = 0;
@@ -503,6 +520,7 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
             since_flush = 0;
             if constexpr (TMEM) {
                 if (k + 1 < p.nk) {  // (the last stage's sums go straight to the epilogue)
+                    const uint32_t taddr = tmem_addr();
 #pragma unroll
                     for (int ch = 0; ch < NCOL / 16; ++ch) {
                         uint32_t t[16];
@@ -541,7 +559,16 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
     }
 
     // ========================= store (a7): lane l of superword j is output sample l*L + j
+    // (the CTA's tile is recomputed here instead of being kept in registers across the hot loop)
+    int b, jt;
+    {
+        int bid = blockIdx.x;
+        asm volatile("" : "+r"(bid));
+        tile_of_cta(p, bid, b, jt);
+    }
+    const int64_t j0 = static_cast<int64_t>(jt) * D_J;
     if constexpr (TMEM) {
+        const uint32_t taddr = tmem_addr();
 #pragma unroll
         for (int ch = 0; ch < NCOL / 16; ++ch) {
             uint32_t t[16];
@@ -571,7 +598,11 @@ __global__ void __launch_bounds__((WD * WJ + 1) * 32, NB) dedisperse_kernel(cons
         }
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         asm volatile("bar.sync 1, %0;" ::"r"((NCW + 1) * 32) : "memory");
-        if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(TCOLS) : "memory");
+        if (warp == 0) {
+            uint32_t tmem;
+            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem) : "r"(bar_full + 960u) : "memory");
+            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(TCOLS) : "memory");
+        }
         return;
     }
 #pragma unroll
@@ -1258,25 +1289,24 @@ const Variant kVariants[] = {
     DD_VARIANT(DD_F32, 1, 1, 8, 16, 1, 16, 0, 1, 2, 0),  // 13
     DD_VARIANT(DD_F32, 1, 1, 8, 4, 4, 8, 0, 1, 2, 0),    // 14
     DD_VARIANT(DD_F32, 1, 1, 8, 1, 16, 4, 0, 1, 4, 0),   // 15 one DM per block: always fits
-    // u4: eight 4-bit lanes per word, LDS.64 superwords of 16 samples, 12 DM warps x 8 superwords,
-    // odd nibbles by LOP3 + LEA.HI on the alu pipe, the whole-word add on the fma pipe (FM = 4)
-    DD_VARIANT(DD_U4, 2, 1, 8, 12, 1, 16, 4, 1, 4, 0),   // 16
-    DD_VARIANT(DD_U4, 2, 1, 8, 12, 1, 8, 4, 1, 4, 0),    // 17
-    DD_VARIANT(DD_U4, 2, 1, 8, 6, 2, 8, 4, 1, 4, 0),     // 18
-    DD_VARIANT(DD_U4, 2, 1, 8, 3, 4, 4, 4, 1, 4, 0),     // 19
-    DD_VARIANT(DD_U4, 2, 1, 4, 3, 4, 4, 4, 1, 4, 0),     // 20
-    DD_VARIANT(DD_U4, 2, 1, 4, 1, 12, 4, 4, 1, 4, 0),    // 21 one DM per block: always fits
+    // u4: eight 4-bit lanes per word, LDS.64 superwords of 16 samples, 11 DM warps x 8 superwords
+    // (12 warps in all = 3 per scheduler: up to 168 registers, the 6 accumulator registers per word
+    // need 156), odd nibbles by LOP3 + LEA.HI on the alu pipe, the whole-word add on the fma pipe
+    DD_VARIANT(DD_U4, 2, 1, 8, 11, 1, 16, 4, 1, 4, 0),   // 16
+    DD_VARIANT(DD_U4, 2, 1, 8, 11, 1, 8, 4, 1, 4, 0),    // 17
+    DD_VARIANT(DD_U4, 2, 1, 8, 5, 2, 8, 4, 1, 4, 0),     // 18
+    DD_VARIANT(DD_U4, 2, 1, 8, 3, 3, 4, 4, 1, 4, 0),     // 19
+    DD_VARIANT(DD_U4, 2, 1, 4, 3, 3, 4, 4, 1, 4, 0),     // 20
+    DD_VARIANT(DD_U4, 2, 1, 4, 1, 11, 4, 4, 1, 4, 0),    // 21 one DM per block: always fits
 #ifdef DD_TUNING
-    DD_VARIANT(DD_U4, 2, 1, 8, 12, 1, 16, 0, 1, 4, 1),   // 22 compiler's choice of shift-and-add
+    DD_VARIANT(DD_U4, 2, 1, 8, 12, 1, 16, 4, 1, 4, 1),   // 22 12 DM warps (128 registers: spills)
     DD_VARIANT(DD_U4, 2, 1, 8, 12, 1, 16, 2, 1, 4, 1),   // 23 SHF + LOP3, both adds on fma
-    DD_VARIANT(DD_U4, 2, 1, 6, 12, 1, 16, 4, 1, 4, 1),   // 24 6 superwords
+    DD_VARIANT(DD_U4, 2, 1, 6, 12, 1, 16, 4, 1, 4, 1),   // 24 12 DM warps x 6 superwords
     DD_VARIANT(DD_U4, 4, 1, 4, 12, 1, 16, 4, 1, 4, 1),   // 25 LDS.128 x 4
-    DD_VARIANT(DD_U4, 4, 1, 3, 12, 1, 16, 4, 1, 4, 1),   // 26 LDS.128 x 3
+    DD_VARIANT(DD_U4, 2, 1, 8, 12, 1, 16, 0, 1, 4, 1),   // 26 compiler's choice of shift-and-add
     DD_VARIANT(DD_U4, 2, 1, 8, 12, 1, 16, 3, 1, 4, 1),   // 27 IMAD.WIDE 64-bit whole-word sum
     DD_VARIANT(DD_U4, 2, 1, 8, 12, 1, 16, 1, 1, 4, 1),   // 28 W as IADD3
-    DD_VARIANT(DD_U4, 2, 1, 8, 8, 1, 16, 4, 1, 4, 1),    // 29 8 DM warps
-    DD_VARIANT(DD_U4, 2, 1, 4, 12, 2, 16, 4, 1, 4, 1),   // 30 24 warps x 4 superwords
-    DD_VARIANT(DD_U4, 2, 1, 8, 11, 1, 16, 4, 1, 4, 1),   // 31 11 DM warps (12 warps in all: 168 registers)
+    DD_VARIANT(DD_U4, 2, 1, 9, 11, 1, 16, 4, 1, 4, 1),   // 29 11 DM warps x 9 superwords
     DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 2, 1, 4, 1),   // r01b shape: accumulators in registers
     DD_VARIANT(DD_U8, 1, 1, 8, 16, 1, 16, 0, 1, 4, 1),   // r01 first shape
     DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 1, 1, 4, 1),   // W on fma instead of O
