@@ -20,7 +20,8 @@ inside the timed region), `roofline` (shared-memory pipe, the binding one) with 
 `roofline_hbm`, `cpu_baseline` (the oracle on the host cores, about 10 s), `kernels_ms`,
 `realtime_factor` (Eq. 10), `time_major` (dd_execute_tm / dd_execute_host_tm / dd_transpose) and
 `time_binning` (dd_bin_time).  Extra workloads: headline_u4 (packed 4-bit), paper52 (the paper's
-section 5.2 plan); --nsamps overrides the block length.
+section 5.2 plan), survey52 (a multi-range binned plan over a time-major block through
+dd_survey_execute_tm: the paper's pipeline real-time factor); --nsamps overrides the block length.
 """
 from __future__ import annotations
 
@@ -543,8 +544,151 @@ def run_ours(args):
     return 0
 
 
+# ------------------------------------------------------------------------- survey pipeline
+def run_survey(args):
+    """--config survey52: a multi-range plan over one time-major block through dd_survey_execute_tm
+    (transpose + time binning + dedispersion of every range, all in the library).  Reports the
+    paper's real-time factor R = t_obs / t_c (Eq. 10: t_c includes transpose and
+    binning, not the host->device copy) beside adds/s; `e2e` adds the copies."""
+    import torch
+    rank, local_rank, world = _dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    sys.stdout.flush()
+    saved_stdout = os.dup(1)
+    os.dup2(2, 1)
+    dist = None
+    if world > 1 or "TORCHELASTIC_RUN_ID" in os.environ:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    from paper_2311_05341_b200 import binding as B, build, shard
+    if rank == 0:
+        build.build()
+    if dist is not None:
+        dist.barrier()
+    sc = W.SURVEYS[args.config]
+    hbm_gbs, _, peak_kind = _peaks()
+    import dataclasses
+    gen = W.Config(sc.name, sc.nchans, sc.nsamps, sc.in_dtype, sc.f_high, sc.chan_bw, sc.tsamp, 1, 0.0,
+                   seed=sc.seed + 1000 * rank, mean=sc.mean, sd=sc.sd)
+    x_tm = W.noise_torch(gen, "cuda").t().contiguous()      # [nsamps][nchans], resident in HBM
+    sv = B.Survey(sc.nchans, sc.nsamps, sc.f_high, sc.chan_bw, sc.tsamp, sc.ranges, sc.in_dtype)
+    adds = sum(n * ol * sc.nchans for n, ol in zip(sv.ndm, sv.out_len))
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        sv.execute_tm(x_tm)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t_host0 = time.perf_counter()
+    e0.record(stream)
+    for _ in range(args.steps):
+        sv.execute_tm(x_tm)
+    e1.record(stream)
+    barrier()
+    t_host1 = time.perf_counter()
+    ms_total = e0.elapsed_time(e1)
+    clocks = sampler.stop(t_host0, t_host1) if rank == 0 else None
+    value, ms_total = shard.job_throughput(float(adds) * args.steps, ms_total, dist, "cuda")
+    ms_step = ms_total / args.steps
+
+    # pre-steps alone: the transpose and each binning (HBM-bound; algorithmic bytes = read + write)
+    def timed(fn, n=3):
+        ts = []
+        for i in range(n + 1):
+            e0.record(stream)
+            fn()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            if i:
+                ts.append(e0.elapsed_time(e1))
+        return float(np.mean(ts))
+    x_cm = torch.empty((sc.nchans, sc.nsamps), dtype=x_tm.dtype, device="cuda")
+    pre = {"transpose_ms": timed(lambda: B.transpose(x_tm, x_cm, sc.nchans, sc.nsamps, sc.in_dtype))}
+    in_bytes = x_tm.numel() * x_tm.element_size()
+    pre["transpose_frac_of_hbm"] = 2.0 * in_bytes / (pre["transpose_ms"] * 1e-3) / 1e9 / hbm_gbs
+    bdt = {W.U8: torch.int16, W.U4: torch.uint8, W.F32: torch.float32}[sc.in_dtype]
+    for f in sorted({r[3] for r in sc.ranges if r[3] > 1}):
+        xb = torch.empty((sc.nchans, sc.nsamps // f), dtype=bdt, device="cuda")
+        ms = timed(lambda: B.bin_time(x_cm, xb, sc.nchans, sc.nsamps, f, sc.in_dtype))
+        pre["bin%d_ms" % f] = ms
+        pre["bin%d_frac_of_hbm" % f] = (in_bytes + xb.numel() * xb.element_size()) / (ms * 1e-3) / 1e9 / hbm_gbs
+        del xb
+    del x_cm
+
+    # end to end: pinned time-major host block -> device, the survey, every output plane -> host
+    h_in = torch.empty(x_tm.shape, dtype=x_tm.dtype).pin_memory()
+    h_in.copy_(x_tm)
+    h_outs = [torch.empty(o.shape, dtype=o.dtype).pin_memory() for o in sv.outs]
+    d_in = torch.empty_like(x_tm)
+
+    def e2e_step():
+        d_in.copy_(h_in, non_blocking=True)
+        outs = sv.execute_tm(d_in)
+        for h, o in zip(h_outs, outs):
+            h.copy_(o, non_blocking=True)
+    e2e_step()
+    barrier()
+    e0.record(stream)
+    for _ in range(3):
+        e2e_step()
+    e1.record(stream)
+    barrier()
+    ms_e2e = e0.elapsed_time(e1)
+    e2e_value, ms_e2e = shard.job_throughput(float(adds) * 3, ms_e2e, dist, "cuda")
+    ms_e2e /= 3
+    e2e_verified = all(bool(torch.equal(h, o.cpu())) for h, o in zip(h_outs, sv.execute_tm(x_tm)))
+    if rank != 0:
+        sv.destroy()
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
+        return 0
+    ranges = [{"dm_start": a, "dm_step": b, "count": n, "bin_factor": f, "out_len": ol, "max_shift": mx,
+               "plan_in_dtype": W.DTYPE_NAME[dt]}
+              for (a, b, n, f), ol, mx, dt in zip(sc.ranges, sv.out_len, sv.max_shift, sv.dtype)]
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None,
+            "dtype": "u8 in; unbinned range: packed u16/u32 integer accumulate; binned ranges: u16 in, u32 accumulate; u32 out",
+            "data": "synthetic",
+            "config": {"workload": sc.name, "nchans": sc.nchans, "nsamps": sc.nsamps, "layout": "time-major",
+                       "f_high_MHz": sc.f_high, "chan_bw_MHz": sc.chan_bw, "tsamp_s": sc.tsamp,
+                       "in_dtype": W.DTYPE_NAME[sc.in_dtype], "ranges": ranges, "adds_per_step": adds,
+                       "l2": "input (%.2f GiB) and outputs exceed the 126 MB L2; no flush needed" % (in_bytes / 2 ** 30)},
+            "api": "dd_survey_execute_tm (transpose + time binning + dedispersion of every range)",
+            "realtime_factor": {"R_eq10": sc.t_obs / (ms_step * 1e-3), "t_obs_s": sc.t_obs, "t_c_ms": ms_step,
+                                "note": "t_c includes transpose and binning, not the host copy (PAPER.md:366-370)"},
+            "pre_steps": pre,
+            "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e, "steps": 3,
+                    "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": sum(h.numel() * 4 for h in h_outs),
+                    "api": "pinned host block -> device copy, dd_survey_execute_tm, every output plane -> pinned host",
+                    "R_eq10_with_copies": sc.t_obs / (ms_e2e * 1e-3), "e2e_verified": e2e_verified},
+            "gpu_launches": args.steps * (1 + len({r[3] for r in sc.ranges if r[3] > 1}) + 2 * len(sc.ranges)),
+            "clocks": clocks}
+    sys.stdout.flush()
+    os.dup2(saved_stdout, 1)
+    print(json.dumps(line), flush=True)
+    sv.destroy()
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
 def _apply_overrides(args):
-    if args.nsamps:
+    if args.nsamps and args.config in W.ALL_CONFIGS:
         import dataclasses
         base = W.ALL_CONFIGS[args.config]
         W.ALL_CONFIGS[args.config] = dataclasses.replace(base, nsamps=args.nsamps,
@@ -556,7 +700,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="headline", choices=list(W.ALL_CONFIGS))
+    ap.add_argument("--config", default="headline", choices=list(W.ALL_CONFIGS) + list(W.SURVEYS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--probe-peaks", action="store_true",
                     help="only run the library's on-chip peak probes (dd_probe) and print them")
@@ -565,6 +709,11 @@ def main():
                          "on the observation length, PAPER.md:287); the line's config says so")
     args = ap.parse_args()
     _apply_overrides(args)
+    if args.config in W.SURVEYS:
+        if args.impl == "reference":   # the oracle arm times single plans only
+            print(json.dumps({"impl": "reference", "unavailable": "survey workloads have no oracle timing arm"}))
+            return 0
+        return run_survey(args)
     if args.impl == "reference":
         return run_reference(args)
     if args.probe_peaks:

@@ -62,8 +62,8 @@ int dd_shift_table_build(int nchans, double f_high_MHz, double chan_bw_MHz, doub
  * of one input block).  Launches no kernel on the data path.
  *   in_dtype: DD_U8 / DD_U16 / DD_F32, or DD_U4 = packed 4-bit samples (the paper's third
  *   precision): two samples per byte, the earlier one in the low nibble,
- *   rows of nsamps/2 bytes, nsamps even; output uint32.  DD_U4 rows are widened to 8-bit
- *   lanes by the pre-pass and then run through the 8-bit kernel.
+ *   rows of nsamps/2 bytes, nsamps even; output uint32.  DD_U4 samples stay packed on chip
+ *   (eight 4-bit lanes per 32-bit shared-memory word) and are summed exactly.
  * Errors (with *out = NULL): DD_ERR_INVALID_ARG (as dd_shift_table_build, plus out == NULL,
  * nsamps <= 0, unknown dtype); DD_ERR_SHIFT_TOO_LARGE (max shift >= nsamps);
  * DD_ERR_OVERFLOW (u8: 255*nchans >= 2^32; u16: 65535*nchans >= 2^32; u4: 15*nchans >= 2^32); DD_ERR_ALLOC;
@@ -134,6 +134,47 @@ int dd_transpose(const void *d_in_tm, void *d_out, int nchans, int64_t nsamps, i
  */
 int dd_bin_time(const void *d_in, void *d_out, int nchans, int64_t nsamps, int factor, int in_dtype,
                 void *cuda_stream);
+
+/*
+ * Multi-range DM survey plans: the pipeline the paper times around its dedispersion kernel --
+ * optional transpose of a time-major block, time binning per DM range, dedispersion of every
+ * range (Table 2, 303-309; t_c of Eq. 10 "includes the time required for
+ * dedispersion, the transpose of the input data (if necessary) and downsampling", 370).
+ *
+ * A range is `count` DM trials dm_start + i*dm_step (one multiply, one add per trial) searched
+ * on the block binned in time by bin_factor (1 = not binned; 2, 4, 8 or 16 as dd_bin_time).
+ * dd_survey_create makes one dd_plan per range -- for a binned range a plan with tsamp*bin_factor,
+ * nsamps/bin_factor and dd_bin_time's output type (DD_U8 -> DD_U16, DD_U4 -> DD_U8, DD_F32 ->
+ * DD_F32) -- and one device buffer per distinct factor.  Errors: as dd_plan_create for any range;
+ * DD_ERR_INVALID_ARG (no ranges, count <= 0, bad factor); DD_ERR_UNSUPPORTED_PLAN (a binned range
+ * of DD_U16 input).  *out = NULL on error.
+ *
+ * dd_survey_execute: d_in DEVICE channel-major [nchans][nsamps]; d_out HOST array of nranges
+ * DEVICE pointers, d_out[r] dense [count_r][out_len_r] (uint32 or float32; sizes from
+ * dd_plan_shift_table(dd_survey_plan(s, r), ...)).  Bins once per distinct factor, then runs every
+ * range, all asynchronously on `cuda_stream`; no allocation.
+ * dd_survey_execute_tm: d_in_tm DEVICE time-major [nsamps][nchans].  Without binned ranges every
+ * range reads it through the fused time-major pre-pass (dd_execute_tm); with binned ranges the
+ * block is transposed once (dd_transpose, into a survey-owned buffer allocated on first use) and
+ * every range reads the channel-major copy.  DD_ERR_UNSUPPORTED_PLAN for DD_U4 with binned ranges.
+ * dd_survey_plan: the plan of range r (owned by the survey; NULL if r is out of range);
+ * dd_survey_range_dtype: the input type of that plan; dd_survey_num_ranges: how many.
+ * dd_survey_destroy: frees everything (waits for the device); NULL is a no-op.
+ */
+typedef struct dd_survey dd_survey;
+typedef struct dd_dm_range {
+    double dm_start, dm_step;
+    int32_t count;
+    int32_t bin_factor;
+} dd_dm_range;
+int dd_survey_create(dd_survey **out, int nchans, int64_t nsamps, double f_high_MHz, double chan_bw_MHz,
+                     double tsamp_s, const dd_dm_range *ranges, int nranges, int in_dtype);
+int dd_survey_num_ranges(const dd_survey *survey);
+const dd_plan *dd_survey_plan(const dd_survey *survey, int range);
+int dd_survey_range_dtype(const dd_survey *survey, int range);
+int dd_survey_execute(dd_survey *survey, const void *d_in, void *const *d_out, void *cuda_stream);
+int dd_survey_execute_tm(dd_survey *survey, const void *d_in_tm, void *const *d_out, void *cuda_stream);
+void dd_survey_destroy(dd_survey *survey);
 
 /*
  * The same transform with HOST buffers: h_in [nchans][nsamps], h_out [ndm][out_len].

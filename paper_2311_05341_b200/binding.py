@@ -30,7 +30,9 @@ INFO = {"D_DM": 0, "D_J": 1, "LANES": 2, "L": 3, "SMEM_BYTES": 4, "GRID": 5, "TH
 SYMBOLS = ("dd_shift_table_build", "dd_plan_create", "dd_plan_shift_table", "dd_execute",
            "dd_execute_host", "dd_execute_host_tm", "dd_execute_tm", "dd_transpose", "dd_bin_time",
            "dd_plan_set_host_chunks", "dd_plan_info", "dd_plan_set_timing", "dd_plan_kernel_times",
-           "dd_probe", "dd_plan_destroy", "dd_strerror", "dd_version")
+           "dd_probe", "dd_plan_destroy", "dd_strerror", "dd_version",
+           "dd_survey_create", "dd_survey_num_ranges", "dd_survey_plan", "dd_survey_range_dtype",
+           "dd_survey_execute", "dd_survey_execute_tm", "dd_survey_destroy")
 
 # dd_probe keys (include/dd.h DD_PROBE_*)
 PROBES = {"SM_COUNT": 0, "SM_CLOCK_MHZ": 1, "LDS32": 2, "LDS64": 3, "LDS128": 4, "IADD3": 5,
@@ -92,6 +94,21 @@ def lib() -> ctypes.CDLL:
         L.dd_strerror.argtypes = [c.c_int]
         L.dd_version.restype = c.c_char_p
         L.dd_version.argtypes = []
+        L.dd_survey_create.restype = c.c_int
+        L.dd_survey_create.argtypes = [c.POINTER(c.c_void_p), c.c_int, c.c_int64, c.c_double, c.c_double,
+                                       c.c_double, c.c_void_p, c.c_int, c.c_int]
+        L.dd_survey_num_ranges.restype = c.c_int
+        L.dd_survey_num_ranges.argtypes = [c.c_void_p]
+        L.dd_survey_plan.restype = c.c_void_p
+        L.dd_survey_plan.argtypes = [c.c_void_p, c.c_int]
+        L.dd_survey_range_dtype.restype = c.c_int
+        L.dd_survey_range_dtype.argtypes = [c.c_void_p, c.c_int]
+        L.dd_survey_execute.restype = c.c_int
+        L.dd_survey_execute.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p]
+        L.dd_survey_execute_tm.restype = c.c_int
+        L.dd_survey_execute_tm.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p]
+        L.dd_survey_destroy.restype = None
+        L.dd_survey_destroy.argtypes = [c.c_void_p]
         _lib = L
     return _lib
 
@@ -279,55 +296,69 @@ def _stream_ptr(stream) -> int:
 BIN_OUT_DTYPE = {DD_U8: DD_U16, DD_U4: DD_U8, DD_F32: DD_F32}   # dd_bin_time widens integer types
 
 
+class _DmRange(ctypes.Structure):
+    _fields_ = [("dm_start", ctypes.c_double), ("dm_step", ctypes.c_double),
+                ("count", ctypes.c_int32), ("bin_factor", ctypes.c_int32)]
+
+
 class Survey:
-    """A multi-range DM survey plan in the style of the paper's Table 2: each
-    range is (dm_start, dm_step, count, bin_factor); ranges with bin_factor > 1 run on the
-    time-binned block (dd_bin_time) with tsamp * bin_factor.  Marshalling and a loop only: one
-    dd_plan per range, one binned device buffer per distinct factor, every step in the
-    library's kernels.  ``execute`` returns one output tensor per range."""
+    """dd_survey_create / dd_survey_execute[_tm] / dd_survey_destroy: a multi-range DM survey plan in
+    the style of the paper's Table 2.  ``ranges`` = (dm_start, dm_step, count,
+    bin_factor) tuples.  Marshalling only: the plans, the binned blocks and the loop over ranges
+    live in the library; this class allocates the output tensors (one per range) and hands their
+    addresses over.  ``execute`` / ``execute_tm`` return those tensors."""
 
     def __init__(self, nchans, nsamps, f_high_MHz, chan_bw_MHz, tsamp_s, ranges, in_dtype):
         import torch
-        self.nchans, self.nsamps, self.in_dtype = int(nchans), int(nsamps), int(in_dtype)
-        self.ranges, self.plans, self.outs, self.binned = [], [], [], {}
-        tdt = {DD_U8: torch.uint8, DD_U16: torch.uint16, DD_F32: torch.float32}
-        try:
-            for dm_start, dm_step, count, factor in ranges:
-                dms = float(dm_start) + np.arange(int(count), dtype=np.float64) * float(dm_step)
-                factor = int(factor)
-                if factor == 1:
-                    dt, ns, ts = self.in_dtype, self.nsamps, float(tsamp_s)
-                else:
-                    if self.in_dtype not in BIN_OUT_DTYPE:
-                        raise DDError(DD_ERR_UNSUPPORTED_PLAN, "Survey: binning of this input type")
-                    dt, ns, ts = BIN_OUT_DTYPE[self.in_dtype], self.nsamps // factor, float(tsamp_s) * factor
-                    if factor not in self.binned:
-                        self.binned[factor] = torch.empty((self.nchans, ns), dtype=tdt[dt], device="cuda")
-                plan = Plan(nchans, ns, f_high_MHz, chan_bw_MHz, ts, dms, dt)
-                self.plans.append(plan)
-                self.ranges.append((dms, factor))
-                odt = torch.float32 if dt == DD_F32 else torch.int32
-                self.outs.append(torch.empty((plan.ndm, plan.out_len), dtype=odt, device="cuda"))
-        except Exception:
-            self.destroy()
-            raise
+        arr = (_DmRange * len(ranges))(*[_DmRange(float(a), float(b), int(n), int(f)) for a, b, n, f in ranges])
+        h = ctypes.c_void_p()
+        rc = lib().dd_survey_create(ctypes.byref(h), int(nchans), int(nsamps), float(f_high_MHz),
+                                    float(chan_bw_MHz), float(tsamp_s), ctypes.cast(arr, ctypes.c_void_p),
+                                    len(ranges), int(in_dtype))
+        if rc != DD_OK:
+            raise DDError(rc, "dd_survey_create")
+        self._h = h
+        self.nranges = int(lib().dd_survey_num_ranges(self._h))
+        self.ndm, self.out_len, self.max_shift, self.dtype, self.outs = [], [], [], [], []
+        for r in range(self.nranges):
+            plan = lib().dd_survey_plan(self._h, r)
+            out_len, mx = ctypes.c_int64(), ctypes.c_int32()
+            rc = lib().dd_plan_shift_table(plan, None, ctypes.byref(out_len), ctypes.byref(mx))
+            if rc != DD_OK:
+                raise DDError(rc, "dd_plan_shift_table")
+            dt = int(lib().dd_survey_range_dtype(self._h, r))
+            self.ndm.append(int(ranges[r][2]))
+            self.out_len.append(int(out_len.value))
+            self.max_shift.append(int(mx.value))
+            self.dtype.append(dt)
+            odt = torch.float32 if dt == DD_F32 else torch.int32
+            self.outs.append(torch.empty((self.ndm[-1], self.out_len[-1]), dtype=odt, device="cuda"))
+        self._ptrs = (ctypes.c_void_p * self.nranges)(*[o.data_ptr() for o in self.outs])
 
     def execute(self, d_in, stream=None):
-        done = set()
-        for plan, (dms, factor), out in zip(self.plans, self.ranges, self.outs):
-            if factor == 1:
-                plan.execute(d_in, out, stream)
-                continue
-            if factor not in done:
-                bin_time(d_in, self.binned[factor], self.nchans, self.nsamps, factor, self.in_dtype, stream)
-                done.add(factor)
-            plan.execute(self.binned[factor], out, stream)
+        rc = lib().dd_survey_execute(self._h, _dev_ptr(d_in), ctypes.cast(self._ptrs, ctypes.c_void_p),
+                                     _stream_ptr(stream))
+        if rc != DD_OK:
+            raise DDError(rc, "dd_survey_execute")
+        return self.outs
+
+    def execute_tm(self, d_in_tm, stream=None):
+        rc = lib().dd_survey_execute_tm(self._h, _dev_ptr(d_in_tm), ctypes.cast(self._ptrs, ctypes.c_void_p),
+                                        _stream_ptr(stream))
+        if rc != DD_OK:
+            raise DDError(rc, "dd_survey_execute_tm")
         return self.outs
 
     def destroy(self):
-        for p in self.plans:
-            p.destroy()
-        self.plans = []
+        if getattr(self, "_h", None) is not None and self._h:
+            lib().dd_survey_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
 
     def __enter__(self):
         return self

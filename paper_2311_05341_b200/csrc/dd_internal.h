@@ -108,6 +108,7 @@ struct BinParams {
     void *out;        // [nchans][nout], nout = nsamps / factor
     int64_t nsamps, nout;
     int64_t out_begin;  // first output column the generic kernel produces (set by launch_bin_time)
+    int64_t row_chunks; // thread blocks per channel row of the row-wise kernels (set by launch_bin_time)
     int nchans, factor;
 };
 

@@ -862,33 +862,38 @@ __global__ void __launch_bounds__(256) interleave_u4_kernel(const InterleavePara
 // Time-major filterbank [nsamps][nchans] (how telescopes write it) -> channel-major
 // [nchans][nsamps] (what Eq. 3 / Alg. 3 index); the paper counts this step
 // in its pipeline time.  HBM-bound: every byte is read once and written once.
-// A CTA moves a tile of TC = 32*P channels x TT = 32*P samples (P = elements per 32-bit word).
+// A CTA moves a tile of TC = 32*P channels x 128 samples (P = elements per 32-bit word; 16 KB).
 // Phase 1: a thread loads P words from P consecutive time rows (coalesced along channels),
-// transposes the P x P elements in registers and stores P words into the transposed
-// shared-memory tile.  Phase 2: rows of that tile (one channel, 32*P samples) go out as
-// coalesced word stores.  Ragged edges and rows that are not 4-byte aligned take an
-// element-wise path through the same tile.
+// sixteen words in flight, transposes the P x P elements in registers and stores P words into
+// the transposed shared-memory tile.  Phase 2: rows of that tile (one channel, 128 samples) go
+// out as coalesced word stores; an output row that does not start on a 4-byte boundary
+// (nsamps not a multiple of 4 bytes) gets its words funnel-shifted into place, the few head and
+// tail bytes stored one by one.  Ragged edge tiles and time rows that are not 4-byte aligned
+// take an element-wise path through the same tile.
 template <typename T>
 __global__ void __launch_bounds__(256) transpose_kernel(const TransposeParams p)
 {
-    constexpr int P = 4 / static_cast<int>(sizeof(T));
-    constexpr int TC = 32 * P, TT = 32 * P;
+    constexpr int E = static_cast<int>(sizeof(T));
+    constexpr int P = 4 / E;
+    constexpr int TC = 32 * P, TT = 128;
+    constexpr int WT = TT / P;  // words per tile row
     // [channel row][word along time], +1 word of pitch; channel c of the tile lives in row
     // phys(c) = (c % P) * 32 + c / P so that the 32 lanes of a phase-1 store (consecutive channel
     // words, same k = c % P) hit 32 different banks
-    __shared__ uint32_t tile[TC][33];
+    __shared__ uint32_t tile[TC][WT + 1];
     auto phys = [](int c) { return (c % P) * 32 + c / P; };
     const T *in = static_cast<const T *>(p.in);
     T *out = static_cast<T *>(p.out);
     const int64_t t0 = static_cast<int64_t>(blockIdx.x) * TT;
     const int c0 = static_cast<int>(blockIdx.y) * TC;
     const bool full = t0 + TT <= p.nsamps && c0 + TC <= p.nchans;
-    const bool in_al = (reinterpret_cast<uintptr_t>(in) & 3u) == 0 && (p.nchans * sizeof(T)) % 4 == 0;
-    const bool out_al = (reinterpret_cast<uintptr_t>(out) & 3u) == 0 && (p.nsamps * sizeof(T)) % 4 == 0;
-    if (full && in_al) {
-        uint32_t rr[4][P];  // all 4*P loads of the thread in flight before any is used
+    const bool in_al = (reinterpret_cast<uintptr_t>(in) & 3u) == 0 && (p.nchans * E) % 4 == 0;
+    const bool out_ok = (reinterpret_cast<uintptr_t>(out) & (E - 1)) == 0;
+    if (full && in_al && out_ok) {
+        constexpr int NU = TT / P / 8;  // groups of P time rows per thread
+        uint32_t rr[NU][P];             // all 16 loads of the thread in flight before any is used
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
+        for (int u = 0; u < NU; ++u) {
             const int q = threadIdx.x + 256 * u;
             const int cg = q & 31, tg = q >> 5;
 #pragma unroll
@@ -896,7 +901,7 @@ __global__ void __launch_bounds__(256) transpose_kernel(const TransposeParams p)
                 rr[u][i] = *reinterpret_cast<const uint32_t *>(in + (t0 + tg * P + i) * p.nchans + c0 + cg * P);
         }
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
+        for (int u = 0; u < NU; ++u) {
             const int q = threadIdx.x + 256 * u;
             const int cg = q & 31, tg = q >> 5;  // word along channels, group of P time rows
             uint32_t r[P];
@@ -916,28 +921,43 @@ __global__ void __launch_bounds__(256) transpose_kernel(const TransposeParams p)
                 tile[cg][tg] = r[0];
             }
         }
-    } else {
-        T *te = reinterpret_cast<T *>(&tile[0][0]);  // element view: row pitch 33 words
-        for (int q = threadIdx.x; q < TC * TT; q += 256) {
-            const int c = q % TC, t = q / TC;
-            T v = 0;
-            if (t0 + t < p.nsamps && c0 + c < p.nchans) v = in[(t0 + t) * p.nchans + c0 + c];
-            te[phys(c) * (33 * P) + t] = v;
+        __syncthreads();
+        // a warp writes one tile row (or WT / 32 warps share one) per step
+        const int64_t pitch_b = p.nsamps * E;
+        unsigned char *tile_out = reinterpret_cast<unsigned char *>(out + static_cast<int64_t>(c0) * p.nsamps + t0);
+#pragma unroll 4
+        for (int q = threadIdx.x; q < TC * WT; q += 256) {
+            const int w = q % WT, r = q / WT;
+            const int c = (r % 32) * P + r / 32;  // inverse of phys
+            unsigned char *row = tile_out + c * pitch_b;
+            const uint32_t e = (0u - static_cast<uint32_t>(reinterpret_cast<uintptr_t>(row))) & 3u;  // head bytes
+            const uint32_t lo = tile[r][w];
+            if (e == 0) {
+                reinterpret_cast<uint32_t *>(row)[w] = lo;
+            } else {
+                if (w < WT - 1) *reinterpret_cast<uint32_t *>(row + e + 4 * w) = __funnelshift_r(lo, tile[r][w + 1], 8 * e);
+                // the row's e head bytes and 4 - e tail bytes: byte i of the first / last word
+                if (w < 4) {
+                    const bool head = static_cast<uint32_t>(w) < e;
+                    const uint32_t word = tile[r][head ? 0 : WT - 1];
+                    row[head ? w : 4 * (WT - 1) + w] = static_cast<unsigned char>(word >> (8 * w));
+                }
+            }
         }
+        return;
+    }
+    T *te = reinterpret_cast<T *>(&tile[0][0]);  // element view: row pitch WT + 1 words
+    for (int q = threadIdx.x; q < TC * TT; q += 256) {
+        const int c = q % TC, t = q / TC;
+        T v = 0;
+        if (t0 + t < p.nsamps && c0 + c < p.nchans) v = in[(t0 + t) * p.nchans + c0 + c];
+        te[phys(c) * ((WT + 1) * P) + t] = v;
     }
     __syncthreads();
-    if (full && out_al) {
-        for (int q = threadIdx.x; q < TC * 32; q += 256) {
-            const int w = q & 31, c = q >> 5;
-            *reinterpret_cast<uint32_t *>(out + static_cast<int64_t>(c0 + c) * p.nsamps + t0 + w * P) = tile[phys(c)][w];
-        }
-    } else {
-        const T *te = reinterpret_cast<const T *>(&tile[0][0]);
-        for (int q = threadIdx.x; q < TC * TT; q += 256) {
-            const int t = q % TT, c = q / TT;
-            if (t0 + t < p.nsamps && c0 + c < p.nchans)
-                out[static_cast<int64_t>(c0 + c) * p.nsamps + t0 + t] = te[phys(c) * (33 * P) + t];
-        }
+    for (int q = threadIdx.x; q < TC * TT; q += 256) {
+        const int t = q % TT, c = q / TT;
+        if (t0 + t < p.nsamps && c0 + c < p.nchans)
+            out[static_cast<int64_t>(c0 + c) * p.nsamps + t0 + t] = te[phys(c) * ((WT + 1) * P) + t];
     }
 }
 
@@ -1175,6 +1195,166 @@ __global__ void __launch_bounds__(256) bin_time_fast_kernel(const BinParams p)
     }
 }
 
+// Integer input whose rows are NOT 16-byte aligned (e.g. 156250-sample rows): a piece is 16 bytes
+// of OUTPUT (an aligned vector store; the first aligned output of a row depends on the row) made
+// from 8*F input bytes, which start at any byte address: 2*F + 1 word loads from the 4-byte
+// aligned address below it, funnel-shifted into place.  Sums are formed inside 32-bit words
+// (pairs of bytes / nibbles, then dp4a).  The outputs of a row before its first and after its
+// last whole piece -- and the row's last piece, whose funnel would read past the row -- are made
+// one by one by one thread per row.  Needs in 4-byte aligned and out aligned to its element.
+template <int MODE, int F>
+__global__ void __launch_bounds__(256) bin_time_rows_kernel(const BinParams p)
+{
+    constexpr int OB = MODE == DD_U4 ? 1 : 2;  // bytes per output
+    constexpr int NO = 16 / OB;                // outputs per piece
+    constexpr int NW = 2 * F;                  // input words per piece (8*F bytes, both types)
+    const int64_t nchunk = p.row_chunks;
+    const int c = static_cast<int>(blockIdx.x / nchunk);
+    const size_t row_bytes = MODE == DD_U4 ? static_cast<size_t>(p.nsamps / 2) : static_cast<size_t>(p.nsamps);
+    const uint8_t *row = static_cast<const uint8_t *>(p.in) + c * row_bytes;
+    uint8_t *orow = static_cast<uint8_t *>(p.out) + static_cast<size_t>(c) * p.nout * OB;
+    int64_t head = static_cast<int64_t>((16u - (reinterpret_cast<uintptr_t>(orow) & 15u)) & 15u) / OB;
+    if (head > p.nout) head = p.nout;
+    int64_t npiece = (p.nout - head) / NO - 1;
+    if (npiece < 0) npiece = 0;
+    const int64_t q0 = static_cast<int64_t>(blockIdx.x % nchunk) * 512 + threadIdx.x;
+    uint32_t w[2][NW + 1];
+    const uint8_t *src[2];
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {  // all loads of both pieces first
+        const int64_t q = q0 + u * 256;
+        if (q >= npiece) continue;
+        const int64_t a = (head + q * NO) * F / (MODE == DD_U4 ? 2 : 1);  // first input byte of the piece
+        src[u] = row + a;
+        const uint32_t *al = reinterpret_cast<const uint32_t *>(reinterpret_cast<uintptr_t>(src[u]) & ~static_cast<uintptr_t>(3));
+#pragma unroll
+        for (int i = 0; i < NW; ++i) w[u][i] = al[i];
+        w[u][NW] = (reinterpret_cast<uintptr_t>(src[u]) & 3u) ? al[NW] : 0u;
+    }
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+        const int64_t q = q0 + u * 256;
+        if (q >= npiece) continue;
+        const uint32_t sh = static_cast<uint32_t>(reinterpret_cast<uintptr_t>(src[u]) & 3u) * 8u;
+        uint32_t o[4];  // the 16 output bytes
+        uint32_t part[NW];  // per input word: sums inside the word
+#pragma unroll
+        for (int i = 0; i < NW; ++i) {
+            const uint32_t x = __funnelshift_r(w[u][i], w[u][i + 1], sh);
+            if (MODE == DD_U4)
+                part[i] = (x & 0x0F0F0F0Fu) + ((x >> 4) & 0x0F0F0F0Fu);  // 4 byte lanes: nibble pairs
+            else
+                part[i] = x;                                            // 4 byte lanes: samples
+        }
+        // byte lanes -> outputs.  G = byte lanes per output: u8 F, u4 F/2.
+        constexpr int G = MODE == DD_U4 ? F / 2 : F;
+        if constexpr (G == 1) {  // u4, F = 2: the byte lanes are the outputs (NW = 4 words = 16 outputs)
+#pragma unroll
+            for (int i = 0; i < 4; ++i) o[i] = part[i];
+        } else if constexpr (G == 2) {  // two outputs per word as 16-bit lanes
+            uint32_t h[NW];
+#pragma unroll
+            for (int i = 0; i < NW; ++i) h[i] = (part[i] & 0x00FF00FFu) + ((part[i] >> 8) & 0x00FF00FFu);
+            if constexpr (OB == 2) {  // u8, F = 2: NW = 4 words of two u16 outputs
+#pragma unroll
+                for (int i = 0; i < 4; ++i) o[i] = h[i];
+            } else {                  // u4, F = 4: NW = 8 words of two outputs -> bytes
+#pragma unroll
+                for (int i = 0; i < 4; ++i) o[i] = __byte_perm(h[2 * i], h[2 * i + 1], 0x6420);
+            }
+        } else {  // G >= 4: an output is the sum of G / 4 whole words' byte lanes (dp4a)
+            constexpr int WPO = G / 4;
+            uint32_t v[NO];
+#pragma unroll
+            for (int k = 0; k < NO; ++k) {
+                uint32_t acc = 0u;
+#pragma unroll
+                for (int i = 0; i < WPO; ++i) acc = __dp4a(part[k * WPO + i], 0x01010101u, acc);
+                v[k] = acc;
+            }
+            if constexpr (OB == 2) {
+#pragma unroll
+                for (int i = 0; i < 4; ++i) o[i] = v[2 * i] | v[2 * i + 1] << 16;
+            } else {
+#pragma unroll
+                for (int i = 0; i < 4; ++i) o[i] = v[4 * i] | v[4 * i + 1] << 8 | v[4 * i + 2] << 16 | v[4 * i + 3] << 24;
+            }
+        }
+        *reinterpret_cast<uint4 *>(orow + (head + q * NO) * OB) = make_uint4(o[0], o[1], o[2], o[3]);
+    }
+    if (blockIdx.x % nchunk == 0 && threadIdx.x < 64) {  // the row's edges, one output per step
+        const int64_t body_end = head + npiece * NO;
+        for (int64_t k = threadIdx.x; k < head + (p.nout - body_end); k += 64) {
+            const int64_t t = k < head ? k : body_end + (k - head);
+            uint32_t sum = 0u;
+            for (int i = 0; i < F; ++i) {
+                const int64_t e = t * F + i;
+                if (MODE == DD_U4) {
+                    const uint32_t b = row[e >> 1];
+                    sum += (e & 1) ? b >> 4 : b & 15u;
+                } else {
+                    sum += row[e];
+                }
+            }
+            if (OB == 2)
+                reinterpret_cast<uint16_t *>(orow)[t] = static_cast<uint16_t>(sum);
+            else
+                orow[t] = static_cast<uint8_t>(sum);
+        }
+    }
+}
+
+// float32: a thread makes four consecutive outputs from 4*F consecutive inputs, all loads first,
+// each output summed in ascending i; VEC = widest vector (floats) the row alignment allows.
+template <int F, int VEC>
+__global__ void __launch_bounds__(256) bin_time_f32_kernel(const BinParams p)
+{
+    const int64_t nchunk = p.row_chunks;
+    const int c = static_cast<int>(blockIdx.x / nchunk);
+    const int64_t o0 = (static_cast<int64_t>(blockIdx.x % nchunk) * 256 + threadIdx.x) * 4;
+    if (o0 >= p.nout) return;
+    const float *row = static_cast<const float *>(p.in) + static_cast<size_t>(c) * p.nsamps + o0 * F;
+    float *orow = static_cast<float *>(p.out) + static_cast<size_t>(c) * p.nout + o0;
+    const int nvalid = p.nout - o0 < 4 ? static_cast<int>(p.nout - o0) : 4;
+    float x[4 * F];
+    if (nvalid == 4) {
+        if constexpr (VEC == 4) {
+#pragma unroll
+            for (int k = 0; k < F; ++k) {
+                const float4 v = reinterpret_cast<const float4 *>(row)[k];
+                x[4 * k] = v.x, x[4 * k + 1] = v.y, x[4 * k + 2] = v.z, x[4 * k + 3] = v.w;
+            }
+        } else if constexpr (VEC == 2) {
+#pragma unroll
+            for (int k = 0; k < 2 * F; ++k) {
+                const float2 v = reinterpret_cast<const float2 *>(row)[k];
+                x[2 * k] = v.x, x[2 * k + 1] = v.y;
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < 4 * F; ++k) x[k] = row[k];
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < 4 * F; ++k) x[k] = k < nvalid * F ? row[k] : 0.f;
+    }
+    float acc[4];
+#pragma unroll
+    for (int o = 0; o < 4; ++o) {
+        acc[o] = 0.f;
+#pragma unroll
+        for (int i = 0; i < F; ++i) acc[o] += x[o * F + i];
+    }
+    if (nvalid == 4 && VEC == 4 && (reinterpret_cast<uintptr_t>(orow) & 15u) == 0) {
+        *reinterpret_cast<float4 *>(orow) = make_float4(acc[0], acc[1], acc[2], acc[3]);
+    } else if (nvalid == 4 && (reinterpret_cast<uintptr_t>(orow) & 7u) == 0) {
+        reinterpret_cast<float2 *>(orow)[0] = make_float2(acc[0], acc[1]);
+        reinterpret_cast<float2 *>(orow)[1] = make_float2(acc[2], acc[3]);
+    } else {
+        for (int o = 0; o < nvalid; ++o) orow[o] = acc[o];
+    }
+}
+
 template <int MODE>
 __global__ void __launch_bounds__(256) bin_time_kernel(const BinParams p)
 {
@@ -1360,20 +1540,57 @@ static void launch_bin_fast(const BinParams &p, unsigned grid, cudaStream_t st)
     }
 }
 
+template <int MODE>
+static void launch_bin_rows(const BinParams &p, unsigned grid, cudaStream_t st)
+{
+    switch (p.factor) {
+    case 2: bin_time_rows_kernel<MODE, 2><<<grid, 256, 0, st>>>(p); break;
+    case 4: bin_time_rows_kernel<MODE, 4><<<grid, 256, 0, st>>>(p); break;
+    case 8: bin_time_rows_kernel<MODE, 8><<<grid, 256, 0, st>>>(p); break;
+    default: bin_time_rows_kernel<MODE, 16><<<grid, 256, 0, st>>>(p); break;
+    }
+}
+
+template <int VEC>
+static void launch_bin_f32(const BinParams &p, unsigned grid, cudaStream_t st)
+{
+    switch (p.factor) {
+    case 2: bin_time_f32_kernel<2, VEC><<<grid, 256, 0, st>>>(p); break;
+    case 4: bin_time_f32_kernel<4, VEC><<<grid, 256, 0, st>>>(p); break;
+    case 8: bin_time_f32_kernel<8, VEC><<<grid, 256, 0, st>>>(p); break;
+    default: bin_time_f32_kernel<16, VEC><<<grid, 256, 0, st>>>(p); break;
+    }
+}
+
 int launch_bin_time(int mode, const BinParams &p_in, void *stream)
 {
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     BinParams p = p_in;
     p.out_begin = 0;
-    if (mode != DD_F32) {
+    p.row_chunks = 1;
+    const uintptr_t ain = reinterpret_cast<uintptr_t>(p.in), aout = reinterpret_cast<uintptr_t>(p.out);
+    if (mode == DD_F32) {
+        if ((ain & 3u) == 0 && (aout & 3u) == 0) {
+            // widest loads every row start allows: the thread's inputs start at multiples of 4*F floats
+            const int vec = (ain & 15u) == 0 && p.nsamps % 4 == 0 ? 4 : ((ain & 7u) == 0 && p.nsamps % 2 == 0 ? 2 : 1);
+            p.row_chunks = (p.nout + 1023) / 1024;
+            const unsigned grid = static_cast<unsigned>(p.row_chunks * p.nchans);
+            if (vec == 4)
+                launch_bin_f32<4>(p, grid, st);
+            else if (vec == 2)
+                launch_bin_f32<2>(p, grid, st);
+            else
+                launch_bin_f32<1>(p, grid, st);
+            return static_cast<int>(cudaGetLastError());
+        }
+    } else {
         // whole 16-byte pieces through the fast kernel when every row (input and output) is
         // suitably aligned; the generic kernel finishes the row tails (or does everything)
         const int NS = mode == DD_U4 ? 32 : 16, OB = mode == DD_U4 ? 1 : 2;
         const int NO = NS / p.factor;
         const size_t row_bytes = mode == DD_U4 ? static_cast<size_t>(p.nsamps / 2) : static_cast<size_t>(p.nsamps);
         const int ost = NO * OB;  // bytes per vector store
-        const bool aligned = (reinterpret_cast<uintptr_t>(p.in) & 15u) == 0 && row_bytes % 16 == 0 &&
-                             (reinterpret_cast<uintptr_t>(p.out) % ost) == 0 &&
+        const bool aligned = (ain & 15u) == 0 && row_bytes % 16 == 0 && (aout % ost) == 0 &&
                              (static_cast<size_t>(p.nout) * OB) % ost == 0;
         const int64_t npiece = p.nout / NO;
         if (aligned && npiece > 0) {
@@ -1383,6 +1600,16 @@ int launch_bin_time(int mode, const BinParams &p_in, void *stream)
             else
                 launch_bin_fast<DD_U4>(p, grid, st);
             p.out_begin = npiece * NO;
+        } else if ((ain & 3u) == 0 && (aout % OB) == 0 && p.nout >= 64) {
+            // rows of any length: aligned output pieces from funnel-shifted input words
+            const int64_t maxpiece = p.nout / (16 / OB) + 1;
+            p.row_chunks = (maxpiece + 511) / 512;
+            const unsigned grid = static_cast<unsigned>(p.row_chunks * p.nchans);
+            if (mode == DD_U8)
+                launch_bin_rows<DD_U8>(p, grid, st);
+            else
+                launch_bin_rows<DD_U4>(p, grid, st);
+            return static_cast<int>(cudaGetLastError());
         }
     }
     if (p.out_begin < p.nout) {
@@ -1401,7 +1628,7 @@ int launch_transpose(int mode, const TransposeParams &p, void *stream)
 {
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const int P = mode == DD_U8 ? 4 : (mode == DD_U16 ? 2 : 1);
-    const dim3 grid(static_cast<unsigned>((p.nsamps + 32 * P - 1) / (32 * P)),
+    const dim3 grid(static_cast<unsigned>((p.nsamps + 127) / 128),
                     static_cast<unsigned>((p.nchans + 32 * P - 1) / (32 * P)));
     if (mode == DD_U8)
         transpose_kernel<uint8_t><<<grid, 256, 0, st>>>(p);

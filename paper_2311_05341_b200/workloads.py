@@ -94,6 +94,42 @@ EXTRA_CONFIGS = {
                                "not in BASELINE.json: SURVEY.md 8(f) rank 2"),
 }
 ALL_CONFIGS = {**CONFIGS, **EXTRA_CONFIGS}
+
+
+@dataclass(frozen=True)
+class SurveyConfig:
+    """A multi-range survey plan over one TIME-MAJOR block (dd_survey_*): the pipeline whose time
+    the paper's real-time factor counts (transpose + binning + dedispersion)."""
+    name: str
+    nchans: int
+    nsamps: int
+    in_dtype: int
+    f_high: float
+    chan_bw: float
+    tsamp: float
+    ranges: tuple          # ((dm_start, dm_step, count, bin_factor), ...)
+    seed: int
+    mean: float
+    sd: float
+    note: str = field(default="", compare=False)
+
+    @property
+    def t_obs(self) -> float:
+        return self.nsamps * self.tsamp
+
+
+SURVEYS = {
+    # The paper's section 5.2 block (8-bit, 8192 channels, 64 us, 10 s, 1250-1550 MHz) delivered
+    # time-major, with a DDplan-style plan: Table 2's three ranges (PAPER.md:303-309; the paper
+    # runs them without binning) followed by one coarser range, each range binned in time by the
+    # factor its DM step has grown by.  The telescope plans of the paper's section 5.5 (DDplan.py
+    # output, PAPER.md:364) are not printed in it; this plan stands in for them.
+    "survey52": SurveyConfig("survey52", 8192, 156250, U8, 1550.0, -300.0 / 8192, 64e-6,
+                             ((0.0, 0.1, 1500, 1), (150.0, 0.2, 750, 2), (300.0, 0.25, 800, 2),
+                              (500.0, 0.5, 1000, 4)),
+                             seed=7, mean=128.0, sd=16.0,
+                             note="PAPER.md section 5.2 block, Table 2 ranges + one, DDplan-style binning"),
+}
 ALL_CONFIGS_NSAMPS = {k: v.nsamps for k, v in ALL_CONFIGS.items()}
 
 TINY_PULSE_T0 = 1000

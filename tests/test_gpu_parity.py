@@ -311,6 +311,7 @@ def test_host_path_pipelined_chunks_match_oracle(B, oracle, dtype, case):
 TM_CASES = [
     # nchans, nsamps: whole tiles, ragged both ways, rows not 4-byte aligned, tiny
     (256, 4096), (130, 5003), (37, 999), (1, 300), (129, 1000), (64, 70001),
+    (128, 30002), (256, 10001),   # full tiles whose output rows start 1, 2 or 3 bytes off a word
 ]
 
 
@@ -470,7 +471,8 @@ def test_large_shift_plans_fall_back_to_smaller_dm_blocks(B, oracle, dtype, case
 
 
 # ------------------------------------------------------------------ time binning (dd_bin_time, R15)
-BIN_SHAPES = [(64, 4096), (37, 5003), (5, 1001), (1, 70), (130, 20000)]
+BIN_SHAPES = [(64, 4096), (37, 5003), (5, 1001), (1, 70), (130, 20000),
+              (12, 156250), (7, 30002)]   # rows that are not 16-byte aligned: the funnel-shift kernel
 
 
 @pytest.mark.parametrize("factor", [2, 4, 8, 16])
@@ -568,6 +570,41 @@ def test_multi_range_survey_matches_oracle_chain(B, oracle, dtype):
                 # here the tolerance form: 1e-4 * sum |in| as for every f32 plan
                 ref, ab = oracle.dedisperse(xb, otab, out_len)
                 assert (np.abs(got.astype(np.float64) - ref) <= 1e-4 * ab).all()
+        # the same survey from the time-major block (dd_survey_execute_tm: one transpose, then the
+        # same binning and plans): identical bits
+        first = [o.clone() for o in outs]
+        for o in outs:
+            o.fill_(0)
+        outs_tm = sv.execute_tm(_torch_in(np.ascontiguousarray(x.T)))
+        torch.cuda.synchronize()
+        for a, b in zip(first, outs_tm):
+            assert torch.equal(a, b)
+
+
+def test_survey_without_binning_time_major_and_errors(B, oracle):
+    """dd_survey_* with no binned range reads the time-major block through the fused pre-pass
+    (Table 2 itself has no binning); argument errors of dd_survey_create."""
+    import torch
+    nchans, nsamps = 72, 20000
+    ranges = [(0.0, 0.5, 30, 1), (15.0, 1.0, 12, 1)]
+    rng = np.random.default_rng(5)
+    x = _rand_input(rng, np.uint8, nchans, nsamps)
+    with B.Survey(nchans, nsamps, 1500.0, -2.0, 64e-6, ranges, B.DD_U8) as sv:
+        assert sv.nranges == 2
+        outs = sv.execute_tm(_torch_in(np.ascontiguousarray(x.T)))
+        torch.cuda.synchronize()
+        for (start, step, count, _), got in zip(ranges, outs):
+            dms = start + np.arange(count) * step
+            otab, omx = oracle.shift_table(nchans, 1500.0, -2.0, 64e-6, dms)
+            assert np.array_equal(got.cpu().numpy().view(np.uint32), oracle.dedisperse(x, otab, nsamps - omx))
+    for bad, status in (([(0.0, 1.0, 10, 3)], B.DD_ERR_INVALID_ARG), ([(0.0, 1.0, 0, 1)], B.DD_ERR_INVALID_ARG),
+                        ([], B.DD_ERR_INVALID_ARG)):
+        with pytest.raises(B.DDError) as e:
+            B.Survey(nchans, nsamps, 1500.0, -2.0, 64e-6, bad, B.DD_U8)
+        assert e.value.status == status
+    with pytest.raises(B.DDError) as e:   # no wider integer type to bin 16-bit samples into
+        B.Survey(nchans, nsamps, 1500.0, -2.0, 64e-6, [(0.0, 1.0, 10, 2)], B.DD_U16)
+    assert e.value.status == B.DD_ERR_UNSUPPORTED_PLAN
 
 
 def test_plans_of_one_shape_with_different_ring_sizes_coexist(B, oracle):
