@@ -233,8 +233,8 @@ class _OracleFacts:
 
 
 def _config_dict(cfg, plan):
-    d = {"workload": cfg.name + ("" if cfg.nsamps == W.ALL_CONFIGS_NSAMPS.get(cfg.name, cfg.nsamps)
-                                 else " (nsamps overridden)"), "nchans": cfg.nchans, "nsamps": cfg.nsamps, "ndm": cfg.ndm,
+    d = {"workload": cfg.name + ("" if (cfg.nsamps, cfg.ndm, cfg.dm_step) == W.ALL_CONFIGS_SHAPE.get(cfg.name)
+                                 else " (nsamps / ndm / dm_step overridden)"), "nchans": cfg.nchans, "nsamps": cfg.nsamps, "ndm": cfg.ndm,
          "dm_step": cfg.dm_step, "f_high_MHz": cfg.f_high, "chan_bw_MHz": cfg.chan_bw,
          "tsamp_s": cfg.tsamp, "in_dtype": W.DTYPE_NAME[cfg.in_dtype],
          "l2": "input (%.2f GiB) and output are each larger than the 126 MB L2; no flush needed"
@@ -688,11 +688,16 @@ def run_survey(args):
 
 
 def _apply_overrides(args):
-    if args.nsamps and args.config in W.ALL_CONFIGS:
-        import dataclasses
+    import dataclasses
+    if args.config not in W.ALL_CONFIGS:
+        return
+    if args.nsamps:
         base = W.ALL_CONFIGS[args.config]
-        W.ALL_CONFIGS[args.config] = dataclasses.replace(base, nsamps=args.nsamps,
-                                                         name=base.name)
+        W.ALL_CONFIGS[args.config] = dataclasses.replace(base, nsamps=args.nsamps, name=base.name)
+    if args.dm_step or args.ndm:   # (single-range configs only)
+        base = W.ALL_CONFIGS[args.config]
+        W.ALL_CONFIGS[args.config] = dataclasses.replace(base, dm_step=args.dm_step or base.dm_step,
+                                                         ndm=args.ndm or base.ndm, name=base.name)
 
 
 def main():
@@ -707,6 +712,9 @@ def main():
     ap.add_argument("--nsamps", type=int, default=0,
                     help="override the config's block length (sanity check: adds/s should not depend "
                          "on the observation length, PAPER.md:287); the line's config says so")
+    ap.add_argument("--dm-step", type=float, default=0.0,
+                    help="override the config's DM step (walks down the DM-block ladder: profiles/r02_ladder.md)")
+    ap.add_argument("--ndm", type=int, default=0, help="override the config's number of DM trials")
     args = ap.parse_args()
     _apply_overrides(args)
     if args.config in W.SURVEYS:

@@ -88,6 +88,13 @@ EXTRA_CONFIGS = {
                       seed=6, mean=128.0, sd=16.0,
                       dm_ranges=((0.0, 0.1, 1500), (150.0, 0.2, 750), (300.0, 0.25, 800)),
                       note="PAPER.md section 5.2 / Table 2 at 8192 channels"),
+    # The large-shift regime (where the paper falls back to its "cache
+    # kernel", up to 4x slower): a 300-400 MHz band at 64 us with a coarse DM step -- the shift
+    # grows by up to 630 samples per trial, so dd_plan_create goes down its DM-block ladder
+    # (3 trials per block, 4 channels per stage instead of 12 and 16).
+    "largeshift": Config("largeshift", 4096, 1 << 18, U8, 400.0, -100.0 / 4096, 64e-6, 264, 2.0,
+                         seed=8, mean=128.0, sd=16.0,
+                         note="large-shift regime, SURVEY.md 8(f) rank 3; not in BASELINE.json"),
     "headline_u4": Config("headline_u4", 8192, 1 << 18, U4, 1500.0, -300.0 / 8192, 64e-6, 1024, 2.0,
                           seed=5, mean=7.5, sd=2.0,
                           note="the headline shape at the paper's 4-bit precision (PAPER.md:295, 424); "
@@ -131,6 +138,7 @@ SURVEYS = {
                              note="PAPER.md section 5.2 block, Table 2 ranges + one, DDplan-style binning"),
 }
 ALL_CONFIGS_NSAMPS = {k: v.nsamps for k, v in ALL_CONFIGS.items()}
+ALL_CONFIGS_SHAPE = {k: (v.nsamps, v.ndm, v.dm_step) for k, v in ALL_CONFIGS.items()}
 
 TINY_PULSE_T0 = 1000
 

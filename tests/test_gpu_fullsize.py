@@ -7,8 +7,8 @@ run per config and kernel variant):
     tile edge the kernel has (lane boundaries k*L, word-tile boundaries, DM-block boundaries,
     first/last sample and DM).  Seconds per config.
   * test_full_output_parity (also marked slow) -- EVERY output element of dd_execute against the
-    oracle's whole plane, default kernel variant, for c2, headline, lowfreq, c3, headline_u4 and
-    paper52 (rows that are not 16-byte aligned).  About a minute of oracle time per config.
+    oracle's whole plane, default kernel variant, for c2, headline, lowfreq, c3, headline_u4,
+    paper52 (rows that are not 16-byte aligned) and largeshift (a lower rung of the DM-block ladder).  About a minute of oracle time per config.
   * test_other_entry_points_equal_device_output_full_size -- dd_execute_host and
     dd_execute_host_tm on their DEFAULT chunk schedule (the one bench.py's e2e leg times) and
     dd_execute_tm must reproduce dd_execute's plane bit for bit (same kernels, same per-output
@@ -133,7 +133,7 @@ def test_full_size_sampled_parity(oracle, golden, name):
         plan.destroy()
 
 
-FULL_OUTPUT_CONFIGS = ["c2", "headline", "lowfreq", "c3", "headline_u4", "paper52"]
+FULL_OUTPUT_CONFIGS = ["c2", "headline", "lowfreq", "c3", "headline_u4", "paper52", "largeshift"]
 
 
 @pytest.mark.slow
@@ -268,3 +268,32 @@ def test_binned_range_full_size(oracle):
         rows = [0, plan.ndm - 1]
         got_rows = out[torch.tensor(rows, device="cuda")].cpu().numpy().view(np.uint32)
         assert np.array_equal(got_rows, oracle.dedisperse(xb, otab[rows], plan.out_len))
+
+
+def test_survey_full_size(oracle):
+    """dd_survey_execute_tm on the survey52 workload (time-major 8192 x 156250 uint8 block, four DM
+    ranges binned by 1, 2, 2, 4; bench.py --config survey52): two complete DM rows of every range
+    against the oracle chain (numpy transpose -> oracle_bin_time -> oracle transform)."""
+    import torch
+    B = _gpu()
+    sc = W.SURVEYS["survey52"]
+    gen = W.Config(sc.name, sc.nchans, sc.nsamps, sc.in_dtype, sc.f_high, sc.chan_bw, sc.tsamp, 1, 0.0,
+                   seed=sc.seed, mean=sc.mean, sd=sc.sd)
+    x = W.noise_torch(gen, "cuda")
+    xh = x.cpu().numpy()
+    x_tm = x.t().contiguous()
+    del x
+    with B.Survey(sc.nchans, sc.nsamps, sc.f_high, sc.chan_bw, sc.tsamp, sc.ranges, sc.in_dtype) as sv:
+        outs = sv.execute_tm(x_tm)
+        torch.cuda.synchronize()
+        binned = {1: xh}
+        for (start, step, count, factor), got, out_len in zip(sc.ranges, outs, sv.out_len):
+            if factor not in binned:
+                binned[factor] = oracle.bin_time(xh, factor)
+            xb = binned[factor]
+            dms = start + np.arange(count, dtype=np.float64) * step
+            otab, omx = oracle.shift_table(sc.nchans, sc.f_high, sc.chan_bw, sc.tsamp * factor, dms)
+            assert out_len == xb.shape[1] - omx
+            rows = [0, count - 1]
+            ref = oracle.dedisperse(xb, otab[rows], out_len)
+            assert np.array_equal(got[torch.tensor(rows, device="cuda")].cpu().numpy().view(np.uint32), ref)

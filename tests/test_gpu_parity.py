@@ -738,3 +738,32 @@ def test_plan_errors_on_gpu(B):
     assert e.value.status == B.DD_ERR_INVALID_ARG
     plan.destroy()
     plan.destroy()  # idempotent
+
+
+def test_runs_beside_a_tensor_core_gemm(B, oracle):
+    """The u8 and u4 kernels park accumulators in tensor memory (tcgen05.alloc sized per shape).  A
+    bf16 GEMM (a tcgen05 / TMEM user) running on another stream at the same time must neither
+    block nor disturb them: results stay bit-exact against the oracle."""
+    import torch
+    rng = np.random.default_rng(77)
+    nchans, nsamps = 600, 60000
+    dms = np.arange(48) * 1.0
+    x8 = rng.integers(0, 256, (nchans, nsamps), dtype=np.uint8)
+    xp = W.pack_u4(rng.integers(0, 16, (nchans, nsamps)).astype(np.uint8))
+    a = torch.randn((4096, 4096), dtype=torch.bfloat16, device="cuda")
+    b = torch.randn((4096, 4096), dtype=torch.bfloat16, device="cuda")
+    side = torch.cuda.Stream()
+    for code, x in ((B.DD_U8, x8), (B.DD_U4, xp)):
+        with B.Plan(nchans, nsamps, 1500.0, -300.0 / nchans, 64e-6, dms, code) as plan:
+            d_in = torch.from_numpy(x).cuda()
+            d_out = torch.full((plan.ndm, plan.out_len), -1, dtype=torch.int32, device="cuda")
+            torch.cuda.synchronize()
+            with torch.cuda.stream(side):
+                for _ in range(40):
+                    c = a @ b
+            for _ in range(6):
+                plan.execute(d_in, d_out)
+            torch.cuda.synchronize()
+            run = oracle.dedisperse_u4 if code == B.DD_U4 else oracle.dedisperse
+            assert np.array_equal(d_out.cpu().numpy().view(np.uint32), run(x, plan.shift_table(), plan.out_len))
+            assert torch.isfinite(c.float()).all()
