@@ -468,20 +468,23 @@ def run_ours(args):
     smem_alg_bytes = adds * smem_b                      # one sample read from shared memory per add
     hbm_alg_bytes = int(cfg.nchans * cfg.nsamps * in_b) + plan.ndm * plan.out_len * 4
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "r02_traffic.csv")  # dram bytes per launch from the committed ncu captures
-    if os.path.exists(tpath) and not args.nsamps:
+    # DRAM bytes (read + write) of one dedisperse_kernel launch from the committed ncu captures of
+    # this kernel (profiles/r02_traffic.csv names the capture; profiles/r02_summary.md the commit)
+    tpath = os.path.join(ROOT, "profiles", "r02_traffic.csv")
+    overridden = (cfg.nsamps, cfg.ndm, cfg.dm_step) != W.ALL_CONFIGS_SHAPE.get(cfg.name)
+    if os.path.exists(tpath) and not overridden:
         with open(tpath) as f:
             for ln in f.read().splitlines()[1:]:
-                k, v = ln.split(",")
-                if k == cfg.name:
-                    traffic = int(v)
+                fld = ln.split(",")
+                if fld[0] == cfg.name:
+                    traffic = int(fld[1])
     share = main_s / (main_s + il_s)
     # The dominant kernel reads one sample from shared memory per add: its binding roofline is the
     # shared-memory pipe (ncu: 90-99 % of peak wavefronts), reported in bytes.
     roofline = {"bound": "smem", "kernel": "dedisperse_kernel",
                 "achieved": smem_alg_bytes / main_s / 1e9, "peak": smem_peak_gbs, "unit": "GB/s",
                 "frac": smem_alg_bytes / main_s / 1e9 / smem_peak_gbs, "traffic": traffic,
-                "traffic_note": "DRAM bytes per launch (ncu, profiles/r01d_summary.md for u8, r01b_summary.md for u16/f32); algorithmic HBM bytes %d"
+                "traffic_note": "DRAM bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r02_traffic.csv, r02_summary.md); algorithmic HBM bytes %d"
                                 % hbm_alg_bytes,
                 "peak_kind": "measured (dd_probe): %.1f B/clk/SM x %d SMs x %.0f MHz; derived (paper Eq. 8) %.0f GB/s"
                              % (smem_b_clk, n_sm, probed["SM_CLOCK_MHZ"], smem_peak_derived),

@@ -452,8 +452,12 @@ LARGE_SHIFT_CASES = [
 @pytest.mark.parametrize("case", LARGE_SHIFT_CASES)
 def test_large_shift_plans_fall_back_to_smaller_dm_blocks(B, oracle, dtype, case):
     """Large DM step x small sampling time (the regime of the paper's 'cache kernel',
-    PAPER.md:153, 380): windows of a 12/32-DM block no longer fit shared memory, the plan
-    must pick a smaller DM block and still match the oracle."""
+    PAPER.md:153, 380): when the windows of a 12/16/32-DM block no longer fit shared memory the
+    plan goes down its ladder (smaller stages first: 8 instead of 16 channels; then smaller DM
+    blocks) and must still match the oracle.  `expect` (last field of a case): 0 = any rung (for
+    8-bit input case 0 still fits the first DM block with 8-channel stages since the flush
+    accumulators moved to tensor memory), 1 = a smaller DM block than the
+    first choice, 2 = the last rung (one DM trial per block)."""
     nchans, nsamps, ndm, step, f_high, band, tsamp, expect = case
     rng = np.random.default_rng([nchans, nsamps, ndm, 77])
     x = _rand_input(rng, dtype, nchans, nsamps)

@@ -79,18 +79,31 @@ def test_config_tables_match_survey(oracle, golden, name):
     assert (np.diff(tab, axis=1) >= 0).all() and (np.diff(tab, axis=0) >= 0).all()
 
 
-def test_table_independent_evaluation_order(oracle):
-    # An independently written numpy evaluation with a DIFFERENT operation order
-    # (common denominator form) gives the same integers wherever no value sits within
-    # 1e-9 of a half-integer.
-    cfg = W.CONFIGS["c2"]
+@pytest.mark.parametrize("name", list(W.CONFIGS))
+def test_table_independent_evaluation_order(oracle, name):
+    # Independently written numpy evaluations in FOUR different double operation orders, and one in
+    # extended precision (numpy longdouble, 64-bit mantissa on x86), give the oracle's integers for
+    # every entry of every config table that does not sit within 1e-9 of a half-integer -- and no
+    # entry of the five tables does: the rounding reading R3 is not fragile.
+    cfg = W.CONFIGS[name]
     tab, _ = oracle.shift_table(cfg.nchans, cfg.f_high, cfg.chan_bw, cfg.tsamp, cfg.dm_list)
-    f = cfg.f_high + np.arange(cfg.nchans) * cfg.chan_bw
-    k = 4148.808 * (cfg.f_high ** 2 - f ** 2) / (f ** 2 * cfg.f_high ** 2)
-    real = np.outer(cfg.dm_list, k / cfg.tsamp)
-    frac = np.abs(real - np.floor(real) - 0.5)
+    C = 4148.808
+    fh, ts, dm = cfg.f_high, cfg.tsamp, cfg.dm_list
+    f = fh + np.arange(cfg.nchans) * cfg.chan_bw
+    orders = [
+        np.outer(dm, C * (fh ** 2 - f ** 2) / (f ** 2 * fh ** 2) / ts),      # common denominator
+        np.outer(dm / ts, C / f ** 2 - C / fh ** 2),                          # constant distributed
+        np.outer(dm * C, (1.0 / f ** 2 - 1.0 / fh ** 2)) / ts,                # DM times constant first
+        np.outer(dm, C * (1.0 / f - 1.0 / fh) * (1.0 / f + 1.0 / fh)) / ts,   # difference of squares
+    ]
+    fl = fh + np.arange(cfg.nchans, dtype=np.longdouble) * np.longdouble(cfg.chan_bw)
+    ext = np.outer(dm.astype(np.longdouble),
+                   np.longdouble(C) * (1 / fl ** 2 - 1 / np.longdouble(fh) ** 2)) / np.longdouble(ts)
+    frac = np.abs(ext - np.floor(ext) - np.longdouble(0.5))
     assert frac.min() > 1e-9
-    assert (np.rint(real).astype(np.int32) == tab).all()
+    assert (np.rint(ext).astype(np.int64) == tab).all()
+    for real in orders:
+        assert (np.rint(real).astype(np.int32) == tab).all()
 
 
 def test_shift_table_rejects_positive_bandwidth(oracle):
