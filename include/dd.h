@@ -69,7 +69,7 @@ int dd_shift_table_build(int nchans, double f_high_MHz, double chan_bw_MHz, doub
  * DD_ERR_OVERFLOW (u8: 255*nchans >= 2^32; u16: 65535*nchans >= 2^32; u4: 15*nchans >= 2^32); DD_ERR_ALLOC;
  * DD_ERR_CUDA; DD_ERR_UNSUPPORTED_DEVICE; DD_ERR_UNSUPPORTED_PLAN.
  * The library reads no environment variable.  (A tuning build, `build.py --tuning`, adds the A/B
- * kernel shapes of profiles/r01_tuning.md and honours DD_FORCE_VARIANT=<n>; never the default.)
+ * kernel shapes of profiles/r02_tuning.md and honours DD_FORCE_VARIANT=<n>; never the default.)
  */
 int dd_plan_create(dd_plan **out, int nchans, int64_t nsamps, double f_high_MHz,
                    double chan_bw_MHz, double tsamp_s, const double *dm_list, int ndm,

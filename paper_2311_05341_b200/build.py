@@ -2,7 +2,7 @@
 
     python -m paper_2311_05341_b200.build [--force] [--verbose] [--tuning]
 
---tuning adds -DDD_TUNING: the A/B kernel shapes of profiles/r01_tuning.md and the
+--tuning adds -DDD_TUNING: the A/B kernel shapes of profiles/r02_tuning.md and the
 DD_FORCE_VARIANT environment variable exist only in such a build (never the default).
 
 The .so is git-ignored and travels to the GPU box with the gpurun snapshot.

@@ -1450,7 +1450,7 @@ struct Variant {
 // always fits.  TUNE == 1 entries exist only in tuning builds (build.py --tuning, -DDD_TUNING)
 // and are reachable through the DD_FORCE_VARIANT environment variable of such a build.
 // u8: LDS.64 superwords, 12 DM warps x 12 superwords, odd-lane adds on the fma pipe and the
-// uint32 flush accumulators parked in tensor memory (FM = 4); profiles/r01_tuning.md.
+// uint32 flush accumulators parked in tensor memory (FM = 4); profiles/r02_tuning.md.
 const Variant kVariants[] = {
     //         mode  VW RD RJ  WD  WJ  CH FM NB OW tune
     DD_VARIANT(DD_U8, 2, 1, 12, 12, 1, 16, 4, 1, 4, 0),  // 0
