@@ -253,7 +253,9 @@ def _tile_string(plan):
 
 # ------------------------------------------------------------------------- measured on-chip peaks
 PROBE_UNITS = {"SM_COUNT": "SMs", "SM_CLOCK_MHZ": "MHz", "LDS32": "B/clk/SM", "LDS64": "B/clk/SM",
-               "LDS128": "B/clk/SM", "TMEM_LD": "B/clk/SM", "TMEM_LD_WITH_LDS": "B/clk/SM (each of TMEM and LDS.64)"}
+               "LDS128": "B/clk/SM", "TMEM_LD": "B/clk/SM", "TMEM_LD_WITH_LDS": "B/clk/SM (each of TMEM and LDS.64)",
+               "F32_ADDS_SMEM_ONLY": "f32 adds/clk/SM", "F32_ADDS_TMEM_4_OF_8": "f32 adds/clk/SM",
+               "F32_ADDS_TMEM_4_OF_8_NO_FILL": "f32 adds/clk/SM"}
 
 
 def measure_peaks(B):

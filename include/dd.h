@@ -258,6 +258,11 @@ int dd_plan_kernel_times(dd_plan *plan, int max_n, float *interleave_ms, float *
  *                                product; LOP3, PRMT, SHF, FADD as named)
  *   DD_PROBE_TMEM_LD             tensor-memory bytes read per clock per SM (tcgen05.ld.32x32b.x8)
  *   DD_PROBE_TMEM_LD_WITH_LDS    the same while the CTA also reads as many bytes with LDS.64
+ *   DD_PROBE_F32_ADDS_*          float32 sample-adds per clock per SM of the accumulate loop a
+ *                                "tensor memory as a second operand store" kernel would run (DESIGN.md
+ *                                section 10), global-memory side left out: every operand from shared memory
+ *                                (SMEM_ONLY, the present kernel's loop), or 4 / 8 of every 8 channels copied
+ *                                into tensor-memory windows first and read from there (TMEM_4_OF_8; _NO_FILL: windows filled once only)
  * Blocking (synchronises the device); allocates and frees a few MB.  Errors: DD_ERR_INVALID_ARG,
  * DD_ERR_UNSUPPORTED_DEVICE, DD_ERR_ALLOC, DD_ERR_CUDA.
  */
@@ -278,7 +283,10 @@ enum {
     DD_PROBE_IDP4A = 13,
     DD_PROBE_SHF = 14,
     DD_PROBE_TMEM_LD = 15,
-    DD_PROBE_TMEM_LD_WITH_LDS = 16
+    DD_PROBE_TMEM_LD_WITH_LDS = 16,
+    DD_PROBE_F32_ADDS_SMEM_ONLY = 17,
+    DD_PROBE_F32_ADDS_TMEM_4_OF_8 = 18,
+    DD_PROBE_F32_ADDS_TMEM_4_OF_8_NO_FILL = 19
 };
 int dd_probe(int what, double *value);
 

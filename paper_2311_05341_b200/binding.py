@@ -37,7 +37,8 @@ SYMBOLS = ("dd_shift_table_build", "dd_plan_create", "dd_plan_shift_table", "dd_
 # dd_probe keys (include/dd.h DD_PROBE_*)
 PROBES = {"SM_COUNT": 0, "SM_CLOCK_MHZ": 1, "LDS32": 2, "LDS64": 3, "LDS128": 4, "IADD3": 5,
           "VIADD16X2": 6, "IMAD": 7, "FADD": 8, "LOP3": 9, "PRMT": 10, "SHIFT_ADD": 11, "IMAD_HI": 12,
-          "IDP4A": 13, "SHF": 14, "TMEM_LD": 15, "TMEM_LD_WITH_LDS": 16}
+          "IDP4A": 13, "SHF": 14, "TMEM_LD": 15, "TMEM_LD_WITH_LDS": 16, "F32_ADDS_SMEM_ONLY": 17,
+          "F32_ADDS_TMEM_4_OF_8": 18, "F32_ADDS_TMEM_4_OF_8_NO_FILL": 19}
 
 _lib = None
 

@@ -174,6 +174,117 @@ __global__ void __launch_bounds__(512, 1) tmem_kernel(uint32_t *sink, long long 
     if (threadIdx.x < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 256;" ::"r"(tb));
 }
 
+// ---------------------------------------------------------------- f32 accumulate fed from two operand stores
+// The inner loop a tensor-memory "second operand store" kernel would run,
+// without its global-memory side: 16 warps, a thread owns T = 33 consecutive outputs of RD = 2 DM
+// trials (lane stride 33 words: conflict-free LDS.32 for any shift).  Per group of 8 channels,
+// NT of them are served from tensor memory: the four warps of a lane quarter first copy NT windows
+// of WCOL = 128 columns (T + shift span of 8 DMs, rounded up) from shared memory into their quarter
+// (LDS.32 + tcgen05.st), meet at a named barrier, then every warp reads its 33 columns per (channel,
+// DM) at a warp-uniform offset (tcgen05.ld x32 + x1); the other 8 - NT channels are read from shared
+// memory, one LDS.32 per add.  Reports adds per clock per SM.  NT = 0 is the present kernel's loop;
+// FILL = false fills the windows once only (the cost of the tensor-memory reads alone).
+template <int NT, bool FILL>
+__global__ void __launch_bounds__(512, 1) hybrid_kernel(uint32_t *sink, long long *cycles)
+{
+    constexpr int T = 33, RD = 2, G = 8, WCOL = 128;
+    extern __shared__ uint32_t sm[];
+    __shared__ uint32_t tmem_base;
+    for (int i = threadIdx.x; i < 16384; i += blockDim.x) sm[i] = __float_as_uint(1.0f + (i & 7));
+    if (threadIdx.x < 32) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(
+            static_cast<uint32_t>(__cvta_generic_to_shared(&tmem_base))));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, quarter = warp & 3, member = warp >> 2;
+    const uint32_t taddr = tmem_base + (static_cast<uint32_t>(32 * quarter) << 16);
+    const uint32_t seg = static_cast<uint32_t>(__cvta_generic_to_shared(sm)) + (quarter * 32 + lane) * T * 4;
+    float acc[RD][T];
+#pragma unroll
+    for (int r = 0; r < RD; ++r)
+#pragma unroll
+        for (int i = 0; i < T; ++i) acc[r][i] = 0.f;
+    uint32_t off = sink[threadIdx.x & 31] & 63u;  // warp-uniform pseudo shifts, unknown to the compiler
+    off = __shfl_sync(0xffffffffu, off, 0);
+    __syncthreads();
+    const long long t0 = clock64();
+#pragma unroll 1
+    for (int it = 0; it < 256; ++it) {
+        if (NT > 0) {
+            // fill: this warp copies window `member` (and member + 4 when NT = 8) of its quarter
+#pragma unroll 1
+            for (int wn = member; wn < NT && (FILL || it == 0); wn += 4) {
+#pragma unroll 2
+                for (int c0 = 0; c0 < WCOL; c0 += 16) {
+                    uint32_t v[16];
+#pragma unroll
+                    for (int i = 0; i < 16; ++i)
+                        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v[i]) : "r"(seg + ((wn * 5 + c0 + i + off) & 1023) * 4));
+                    asm volatile(
+                        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(
+                            taddr + wn * WCOL + c0),
+                        "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]),
+                        "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]));
+                }
+            }
+            asm volatile("tcgen05.wait::st.sync.aligned;");
+            asm volatile("tcgen05.fence::before_thread_sync;");
+            asm volatile("bar.sync %0, 128;" ::"r"(1 + quarter));
+            asm volatile("tcgen05.fence::after_thread_sync;");
+#pragma unroll 1
+            for (int wn = 0; wn < NT; ++wn)
+#pragma unroll
+                for (int r = 0; r < RD; ++r) {
+                    const uint32_t col = taddr + wn * WCOL + ((off + 7 * r + wn) & 63u);
+                    // 33 columns as 16 + 16 + 1 (a 32-column load would need 33 more live registers)
+                    uint32_t y[2][16], y32;
+#pragma unroll
+                    for (int h = 0; h < 2; ++h)
+                        asm volatile(
+                            "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                            : "=r"(y[h][0]), "=r"(y[h][1]), "=r"(y[h][2]), "=r"(y[h][3]), "=r"(y[h][4]), "=r"(y[h][5]),
+                              "=r"(y[h][6]), "=r"(y[h][7]), "=r"(y[h][8]), "=r"(y[h][9]), "=r"(y[h][10]), "=r"(y[h][11]),
+                              "=r"(y[h][12]), "=r"(y[h][13]), "=r"(y[h][14]), "=r"(y[h][15])
+                            : "r"(col + 16 * h));
+                    asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(y32) : "r"(col + 32));
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) acc[r][i] += __uint_as_float(y[i >> 4][i & 15]);
+                    acc[r][32] += __uint_as_float(y32);
+                }
+            // the windows may be overwritten only after every warp of the quarter has read them
+            asm volatile("tcgen05.fence::before_thread_sync;");
+            asm volatile("bar.sync %0, 128;" ::"r"(5 + quarter));
+        }
+#pragma unroll
+        for (int ch = NT; ch < G; ++ch)
+#pragma unroll
+            for (int r = 0; r < RD; ++r) {
+                const uint32_t a = seg + ((ch * 11 + r * 3 + off) & 63u) * 4;
+#pragma unroll
+                for (int i = 0; i < T; ++i) {
+                    uint32_t x;
+                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(x) : "r"(a + i * 4));
+                    acc[r][i] += __uint_as_float(x);
+                }
+            }
+    }
+    __syncthreads();
+    const long long t1 = clock64();
+    float s = 0.f;
+#pragma unroll
+    for (int r = 0; r < RD; ++r)
+#pragma unroll
+        for (int i = 0; i < T; ++i) s += acc[r][i];
+    sink[blockIdx.x * blockDim.x + threadIdx.x] = __float_as_uint(s);
+    if (threadIdx.x == 0) cycles[blockIdx.x] = t1 - t0;
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    if (threadIdx.x < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base));
+}
+
 struct Scratch {
     uint32_t *sink = nullptr;
     long long *cycles = nullptr;
@@ -227,6 +338,21 @@ int tmem_rate(Scratch &s, double *out)
     const int rc = median_cycles(s, [&] { tmem_kernel<MODE><<<s.nsm, 512, 32768>>>(s.sink, s.cycles); }, &cyc);
     // per iteration a thread reads 8 words from TMEM (and, MODE 1, 8 words from shared memory)
     if (rc == DD_OK) *out = 512.0 * kIter * 32 / cyc;
+    return rc;
+}
+
+template <int NT, bool FILL>
+int hybrid_rate(Scratch &s, double *out)
+{
+    double cyc = 0;
+    if (cudaFuncSetAttribute(reinterpret_cast<const void *>(hybrid_kernel<NT, FILL>), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             65536 + 8192) != cudaSuccess)
+        return DD_ERR_CUDA;
+    if (cudaMemset(s.cycles, 0, static_cast<size_t>(s.nsm) * sizeof(long long)) != cudaSuccess) return DD_ERR_CUDA;
+    const int rc = median_cycles(s, [&] { hybrid_kernel<NT, FILL><<<s.nsm, 512, 65536 + 8192>>>(s.sink, s.cycles); }, &cyc);
+    if (rc == DD_OK && (cudaGetLastError() != cudaSuccess || cyc <= 0)) return DD_ERR_CUDA;
+    // per iteration a thread performs 8 channels x 2 DM trials x 33 adds
+    if (rc == DD_OK) *out = 512.0 * 256 * 8 * 2 * 33 / cyc;
     return rc;
 }
 
@@ -295,6 +421,9 @@ extern "C" int dd_probe(int what, double *value)
     case DD_PROBE_SHF: return lane_rate<DD_PROBE_SHF>(s, value);
     case DD_PROBE_TMEM_LD: return tmem_rate<0>(s, value);
     case DD_PROBE_TMEM_LD_WITH_LDS: return tmem_rate<1>(s, value);
+    case DD_PROBE_F32_ADDS_SMEM_ONLY: return hybrid_rate<0, true>(s, value);
+    case DD_PROBE_F32_ADDS_TMEM_4_OF_8: return hybrid_rate<4, true>(s, value);
+    case DD_PROBE_F32_ADDS_TMEM_4_OF_8_NO_FILL: return hybrid_rate<4, false>(s, value);
     default: return DD_ERR_INVALID_ARG;
     }
 }
