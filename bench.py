@@ -368,6 +368,12 @@ def run_ours(args):
     ms_e2e /= e2e_steps
     h2d = h_in.numel() * h_in.element_size()
     d2h = h_out.numel() * h_out.element_size()
+    # where the end-to-end time goes: per chunk of the last call, when its input had arrived, its
+    # pre-pass and main kernel had finished and its output was back on the host (ms after the start)
+    tl = plan.host_timeline()
+    e2e_timeline = [{"out_begin": int(o), "h2d_done_ms": round(float(a), 2), "prepass_done_ms": round(float(b), 2),
+                     "main_done_ms": round(float(c), 2), "d2h_done_ms": round(float(d), 2)}
+                    for o, a, b, c, d in zip(*tl)]
     # the timed host path must reproduce the device-resident plane bit for bit (same kernels, same
     # per-output summation order -- float32 too); tests/ tie that plane to the oracle
     plan.execute(x, out)
@@ -536,7 +542,7 @@ def run_ours(args):
             "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e,
                     "steps": e2e_steps, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "api": "dd_execute_host (pinned host buffers, default chunk schedule)",
-                    "e2e_verified": e2e_verified},
+                    "e2e_verified": e2e_verified, "timeline": e2e_timeline},
             "gpu_launches": args.steps * plan.info("LAUNCHES"),
             "clocks": clocks}
     sys.stdout.flush()

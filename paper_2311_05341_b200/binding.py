@@ -29,7 +29,7 @@ INFO = {"D_DM": 0, "D_J": 1, "LANES": 2, "L": 3, "SMEM_BYTES": 4, "GRID": 5, "TH
 # every symbol include/dd.h declares (tests check the .so exports all of them)
 SYMBOLS = ("dd_shift_table_build", "dd_plan_create", "dd_plan_shift_table", "dd_execute",
            "dd_execute_host", "dd_execute_host_tm", "dd_execute_tm", "dd_transpose", "dd_bin_time",
-           "dd_plan_set_host_chunks", "dd_plan_info", "dd_plan_set_timing", "dd_plan_kernel_times",
+           "dd_plan_set_host_chunks", "dd_plan_host_timeline", "dd_plan_info", "dd_plan_set_timing", "dd_plan_kernel_times",
            "dd_probe", "dd_plan_destroy", "dd_strerror", "dd_version",
            "dd_survey_create", "dd_survey_num_ranges", "dd_survey_plan", "dd_survey_range_dtype",
            "dd_survey_execute", "dd_survey_execute_tm", "dd_survey_destroy")
@@ -81,6 +81,8 @@ def lib() -> ctypes.CDLL:
         L.dd_transpose.argtypes = [c.c_void_p, c.c_void_p, c.c_int, c.c_int64, c.c_int, c.c_void_p]
         L.dd_plan_set_host_chunks.restype = c.c_int
         L.dd_plan_set_host_chunks.argtypes = [c.c_void_p, c.c_int]
+        L.dd_plan_host_timeline.restype = c.c_int
+        L.dd_plan_host_timeline.argtypes = [c.c_void_p, c.c_int, c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p]
         L.dd_plan_info.restype = c.c_int64
         L.dd_plan_info.argtypes = [c.c_void_p, c.c_int]
         L.dd_plan_set_timing.restype = c.c_int
@@ -231,6 +233,16 @@ class Plan:
         rc = lib().dd_plan_set_host_chunks(self._h, int(nchunks))
         if rc != DD_OK:
             raise DDError(rc, "dd_plan_set_host_chunks")
+
+    # -- dd_plan_host_timeline
+    def host_timeline(self, max_chunks: int = 16):
+        """Per chunk of the latest execute_host[_tm]: (out_begin, h2d_ms, pre_ms, main_ms, d2h_ms) arrays."""
+        ob = np.zeros(max_chunks, dtype=np.int64)
+        t = [np.zeros(max_chunks, dtype=np.float32) for _ in range(4)]
+        n = lib().dd_plan_host_timeline(self._h, int(max_chunks), ob.ctypes.data, *[a.ctypes.data for a in t])
+        if n < 0:
+            raise DDError(n, "dd_plan_host_timeline")
+        return (ob[:n].copy(),) + tuple(a[:n].copy() for a in t)
 
     # -- dd_plan_set_timing / dd_plan_kernel_times
     def set_timing(self, on: bool) -> None:

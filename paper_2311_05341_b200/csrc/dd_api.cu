@@ -30,6 +30,9 @@ struct dd_plan {
     int host_chunks = 0;  // dd_plan_set_host_chunks: 0 = default tapered schedule, n = n equal chunks
     cudaStream_t st_h2d = nullptr, st_d2h = nullptr, st_pre = nullptr, st_main2 = nullptr;
     cudaEvent_t ev_in[kHostChunks + 1] = {}, ev_done[kHostChunks + 1] = {}, ev_pre[kHostChunks + 1] = {};
+    cudaEvent_t ev_out[kHostChunks + 1] = {};  // chunk g's device->host copy has finished
+    int last_chunks = 0;             // chunks of the latest dd_execute_host[_tm] call
+    int64_t last_edge[kHostChunks + 1] = {};
     uint32_t *d_X2 = nullptr;  // second chunk workspace: chunk g+1 is interleaved while chunk g is dedispersed
     size_t x2_bytes = 0;
     // optional per-kernel timing (dd_plan_set_timing): ring of event triples
@@ -69,6 +72,7 @@ void free_device(dd_plan *p)
             for (cudaEvent_t e : p->ev_in) cudaEventDestroy(e);
             for (cudaEvent_t e : p->ev_done) cudaEventDestroy(e);
             for (cudaEvent_t e : p->ev_pre) cudaEventDestroy(e);
+            for (cudaEvent_t e : p->ev_out) cudaEventDestroy(e);
             cudaStreamDestroy(p->st_h2d);
             cudaStreamDestroy(p->st_d2h);
             cudaStreamDestroy(p->st_pre);
@@ -430,10 +434,13 @@ static int make_host_objects(dd_plan *plan)
     if (plan->host_made) return DD_OK;
     constexpr int NE = dd_plan::kHostChunks + 1;
     cudaStream_t s[4] = {};
-    cudaEvent_t e[3 * NE] = {};
+    cudaEvent_t e[4 * NE] = {};
     bool ok = true;
+    // (Giving the pre-pass stream the highest priority makes the pre-pass of chunk g+1 run beside
+    // chunk g's main kernel instead of in its tail -- dd_plan_host_timeline shows it -- but the
+    // main kernel slows down by as much: the end-to-end time did not move, so priorities are equal.)
     for (cudaStream_t &x : s) ok = ok && cudaStreamCreateWithFlags(&x, cudaStreamNonBlocking) == cudaSuccess;
-    for (cudaEvent_t &x : e) ok = ok && cudaEventCreateWithFlags(&x, cudaEventDisableTiming) == cudaSuccess;
+    for (cudaEvent_t &x : e) ok = ok && cudaEventCreate(&x) == cudaSuccess;  // timed: dd_plan_host_timeline
     if (!ok) {
         for (cudaStream_t x : s)
             if (x) cudaStreamDestroy(x);
@@ -450,6 +457,7 @@ static int make_host_objects(dd_plan *plan)
         plan->ev_in[g] = e[g];
         plan->ev_pre[g] = e[NE + g];
         plan->ev_done[g] = e[2 * NE + g];
+        plan->ev_out[g] = e[3 * NE + g];
     }
     plan->host_made = true;
     return DD_OK;
@@ -617,12 +625,41 @@ static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void 
                               static_cast<size_t>(o1 - o0) * 4, plan->ndm, cudaMemcpyDeviceToHost,
                               plan->st_d2h) != cudaSuccess)
             return fail(DD_ERR_CUDA);
+        cudaEventRecord(plan->ev_out[g], plan->st_d2h);
     }
+    plan->last_chunks = G;
+    for (int g = 0; g <= G; ++g) plan->last_edge[g] = edge[g];
     // every main kernel precedes a copy on st_d2h; the caller's stream also waits for the odd chunks
     if (G > 1) cudaStreamWaitEvent(st, plan->ev_done[((G - 1) & 1) ? G - 1 : G - 2], 0);
     if (cudaStreamSynchronize(plan->st_d2h) != cudaSuccess) return fail(DD_ERR_CUDA);
     if (cudaStreamSynchronize(st) != cudaSuccess) return fail(DD_ERR_CUDA);
     return DD_OK;
+}
+
+int dd_plan_host_timeline(dd_plan *plan, int max_chunks, int64_t *out_begin, float *h2d_ms, float *pre_ms,
+                          float *main_ms, float *d2h_ms)
+{
+    if (!plan || max_chunks < 0) return DD_ERR_INVALID_ARG;
+    if (!plan->host_made || plan->last_chunks == 0) return 0;
+    const int G = plan->last_chunks < max_chunks ? plan->last_chunks : max_chunks;
+    // ev_done[last_chunks] was recorded on the caller's stream when the call started
+    const cudaEvent_t t0 = plan->ev_done[plan->last_chunks];
+    for (int g = 0; g < G; ++g) {
+        float a = 0.f, b = 0.f, c = 0.f, d = 0.f;
+        if (cudaEventElapsedTime(&a, t0, plan->ev_in[g]) != cudaSuccess ||
+            cudaEventElapsedTime(&b, t0, plan->ev_pre[g]) != cudaSuccess ||
+            cudaEventElapsedTime(&c, t0, plan->ev_done[g]) != cudaSuccess ||
+            cudaEventElapsedTime(&d, t0, plan->ev_out[g]) != cudaSuccess) {
+            cudaGetLastError();
+            return DD_ERR_CUDA;
+        }
+        if (out_begin) out_begin[g] = plan->last_edge[g];
+        if (h2d_ms) h2d_ms[g] = a;
+        if (pre_ms) pre_ms[g] = b;
+        if (main_ms) main_ms[g] = c;
+        if (d2h_ms) d2h_ms[g] = d;
+    }
+    return G;
 }
 
 int64_t dd_plan_info(const dd_plan *plan, int what)
