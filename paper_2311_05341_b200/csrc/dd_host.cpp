@@ -144,14 +144,17 @@ bool build_tiling(const KernelShape &shape, int variant, const int32_t *table, i
     // num_sms/nb j tiles touches about nb * span + (num_sms/nb) * tile bytes of X, where tile =
     // one j tile of every channel and span = what one more DM block adds to the staged windows
     // (the shift difference across the block, summed over channels).  Minimal at
-    // nb = sqrt(num_sms * tile / span); panels are made equal.
+    // nb = sqrt(num_sms * tile / span) if the CTAs of a wave stay in step; they drift, and the
+    // measured minimum of the DRAM traffic sits at 0.65-1.0 of that (profiles/r02_tuning.md:
+    // lowfreq 8 where the model says 12, headline 15-22 for 18, c3 16 for 16), so 0.7 of it is
+    // taken; panels are made equal.
     {
         double span = 0.0;
         for (int c = 0; c < nchans; ++c)
             span += static_cast<double>(table[static_cast<size_t>(ndm - 1) * nchans + c] - table[c]);
         span = span * S / t->ndb;
         const double tile = static_cast<double>(t->nch_pad) * D_J * S;
-        double nb = span > 0.0 ? std::sqrt(static_cast<double>(num_sms) * tile / span) : t->ndb;
+        double nb = span > 0.0 ? 0.7 * std::sqrt(static_cast<double>(num_sms) * tile / span) : t->ndb;
         if (nb < 1.0) nb = 1.0;
         if (nb > t->ndb) nb = t->ndb;
         const int npanel = std::max(1, static_cast<int>(std::lround(t->ndb / nb)));
