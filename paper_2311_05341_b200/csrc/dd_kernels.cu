@@ -1493,6 +1493,9 @@ const Variant kVariants[] = {
     DD_VARIANT(DD_U8, 2, 1, 6, 12, 1, 32, 0, 1, 4, 1),   // all adds on alu
     DD_VARIANT(DD_U16, 1, 2, 8, 16, 1, 16, 0, 1, 4, 1),  // r01b shape: 2 DMs x 8 words
     DD_VARIANT(DD_F32, 1, 2, 8, 16, 1, 16, 0, 1, 4, 1),  // 32-bit offsets
+    DD_VARIANT(DD_U8, 2, 1, 14, 12, 1, 16, 4, 1, 4, 1),  // 36 12 DM warps x 14 superwords
+    DD_VARIANT(DD_U8, 2, 1, 16, 11, 1, 16, 4, 1, 4, 1),  // 37 11 DM warps x 16 superwords
+    DD_VARIANT(DD_U8, 2, 1, 14, 11, 1, 16, 4, 1, 4, 1),  // 38 11 DM warps x 14 superwords
 #endif
 };
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
