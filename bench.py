@@ -384,8 +384,14 @@ def run_ours(args):
 
     # ---- time-major input: transpose pre-step + the same path
     tm = None
-    if rank == 0 and cfg.in_dtype != W.U4:  # (the bench has no time-major 4-bit generator)
-        x_tm = x.t().contiguous()
+    if rank == 0:
+        if cfg.in_dtype == W.U4:
+            # repack along channels (reading R16): unpack, transpose, pack pairs of channels
+            v = torch.stack((x & 15, x >> 4), dim=2).reshape(cfg.nchans, cfg.nsamps).t().contiguous()
+            x_tm = (v[:, 0::2] | (v[:, 1::2] << 4)).contiguous()
+            del v
+        else:
+            x_tm = x.t().contiguous()
         x_cm = torch.empty_like(x)
         tms, tot = [], []
         plan.set_timing(True)

@@ -111,8 +111,9 @@ int dd_execute_tm(const dd_plan *plan, const void *d_in_tm, void *d_out, void *c
 /*
  * Stand-alone transpose: time-major d_in_tm [nsamps][nchans] -> channel-major d_out
  * [nchans][nsamps] (the layout dd_execute, dd_execute_host and dd_bin_time take), both DEVICE,
- * dtype DD_U8 / DD_U16 / DD_F32.  Asynchronous on the stream, no allocation.
- * Errors: DD_ERR_INVALID_ARG, DD_ERR_UNSUPPORTED_PLAN (DD_U4), DD_ERR_CUDA.
+ * dtype DD_U8 / DD_U16 / DD_F32, or DD_U4: rows of nchans/2 bytes (even channel in the low nibble) ->
+ * rows of nsamps/2 bytes (earlier sample in the low nibble); nchans and nsamps even.
+ * Asynchronous on the stream, no allocation.  Errors: DD_ERR_INVALID_ARG, DD_ERR_CUDA.
  */
 int dd_transpose(const void *d_in_tm, void *d_out, int nchans, int64_t nsamps, int dtype,
                  void *cuda_stream);
@@ -156,7 +157,7 @@ int dd_bin_time(const void *d_in, void *d_out, int nchans, int64_t nsamps, int f
  * dd_survey_execute_tm: d_in_tm DEVICE time-major [nsamps][nchans].  Without binned ranges every
  * range reads it through the fused time-major pre-pass (dd_execute_tm); with binned ranges the
  * block is transposed once (dd_transpose, into a survey-owned buffer allocated on first use) and
- * every range reads the channel-major copy.  DD_ERR_UNSUPPORTED_PLAN for DD_U4 with binned ranges.
+ * every range reads the channel-major copy.  DD_ERR_UNSUPPORTED_PLAN for DD_U4 with an odd nchans.
  * dd_survey_plan: the plan of range r (owned by the survey; NULL if r is out of range);
  * dd_survey_range_dtype: the input type of that plan; dd_survey_num_ranges: how many.
  * dd_survey_destroy: frees everything (waits for the device); NULL is a no-op.

@@ -345,8 +345,8 @@ int dd_transpose(const void *d_in_tm, void *d_out, int nchans, int64_t nsamps, i
                  void *cuda_stream)
 {
     if (!d_in_tm || !d_out || nchans <= 0 || nsamps <= 0) return DD_ERR_INVALID_ARG;
-    if (dtype == DD_U4) return DD_ERR_UNSUPPORTED_PLAN;
-    if (dtype != DD_U8 && dtype != DD_U16 && dtype != DD_F32) return DD_ERR_INVALID_ARG;
+    if (dtype != DD_U8 && dtype != DD_U16 && dtype != DD_F32 && dtype != DD_U4) return DD_ERR_INVALID_ARG;
+    if (dtype == DD_U4 && ((nchans & 1) || (nsamps & 1))) return DD_ERR_INVALID_ARG;  // whole bytes both ways
     dd::TransposeParams tp;
     tp.in = d_in_tm;
     tp.out = d_out;

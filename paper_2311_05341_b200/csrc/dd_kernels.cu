@@ -961,6 +961,91 @@ __global__ void __launch_bounds__(256) transpose_kernel(const TransposeParams p)
     }
 }
 
+// Packed 4-bit: time-major [nsamps][nchans/2 bytes] (even channel of a byte in the low nibble,
+// reading R16) -> channel-major [nchans][nsamps/2 bytes] (earlier sample in the low nibble, R14).
+// A CTA moves 256 channels x 256 samples.  Two time rows are first merged nibble-wise into the
+// bytes of the even channels and of the odd channels ((t, t+1) of one channel = one output byte);
+// what is left is the byte transpose of transpose_kernel<uint8_t>, once per channel parity.
+__global__ void __launch_bounds__(256) transpose_u4_kernel(const TransposeParams p)
+{
+    constexpr int TC = 256, TU = 128;  // channels, output bytes (pairs of samples) per tile
+    constexpr int WT = TU / 4;         // words per tile row
+    __shared__ uint32_t tile[TC][WT + 1];  // row phys(c) = (c % 8) * 32 + c / 8
+    const uint8_t *in = static_cast<const uint8_t *>(p.in);
+    uint8_t *out = static_cast<uint8_t *>(p.out);
+    const int64_t in_pitch = p.nchans / 2, out_pitch = p.nsamps / 2;  // bytes per input / output row
+    const int64_t u0 = static_cast<int64_t>(blockIdx.x) * TU;         // first output byte column
+    const int c0 = static_cast<int>(blockIdx.y) * TC;
+    const bool full = 2 * (u0 + TU) <= p.nsamps && c0 + TC <= p.nchans;
+    const bool in_al = (reinterpret_cast<uintptr_t>(in) & 3u) == 0 && in_pitch % 4 == 0;
+    if (full && in_al) {
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {  // 2 x 2 groups of (word of 8 channels) x (4 output bytes)
+            uint32_t rr[2][8];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const int q = threadIdx.x + 256 * (2 * half + u);
+                const int cg = q & 31, ug = q >> 5;
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+                    rr[u][i] = *reinterpret_cast<const uint32_t *>(in + (2 * u0 + 8 * ug + i) * in_pitch + c0 / 2 + cg * 4);
+            }
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                const int q = threadIdx.x + 256 * (2 * half + u);
+                const int cg = q & 31, ug = q >> 5;
+                uint32_t ev[4], od[4];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const uint32_t a = rr[u][2 * i], b = rr[u][2 * i + 1];  // samples 2k and 2k+1 of 8 channels
+                    ev[i] = (a & 0x0F0F0F0Fu) | ((b & 0x0F0F0F0Fu) << 4);
+                    od[i] = ((a >> 4) & 0x0F0F0F0Fu) | (b & 0xF0F0F0F0u);
+                }
+#pragma unroll
+                for (int par = 0; par < 2; ++par) {
+                    const uint32_t *x = par ? od : ev;  // byte j of x[i]: channel 8 cg + 2 j + par, output byte 4 ug + i
+                    const uint32_t a = __byte_perm(x[0], x[1], 0x5140), b = __byte_perm(x[0], x[1], 0x7362);
+                    const uint32_t c = __byte_perm(x[2], x[3], 0x5140), d = __byte_perm(x[2], x[3], 0x7362);
+                    tile[(0 + par) * 32 + cg][ug] = __byte_perm(a, c, 0x5410);
+                    tile[(2 + par) * 32 + cg][ug] = __byte_perm(a, c, 0x7632);
+                    tile[(4 + par) * 32 + cg][ug] = __byte_perm(b, d, 0x5410);
+                    tile[(6 + par) * 32 + cg][ug] = __byte_perm(b, d, 0x7632);
+                }
+            }
+        }
+        __syncthreads();
+        unsigned char *tile_out = out + static_cast<int64_t>(c0) * out_pitch + u0;
+#pragma unroll 4
+        for (int q = threadIdx.x; q < TC * WT; q += 256) {
+            const int w = q % WT, r = q / WT;
+            const int c = (r % 32) * 8 + r / 32;  // inverse of phys
+            unsigned char *row = tile_out + c * out_pitch;
+            const uint32_t e = (0u - static_cast<uint32_t>(reinterpret_cast<uintptr_t>(row))) & 3u;  // head bytes
+            const uint32_t lo = tile[r][w];
+            if (e == 0) {
+                reinterpret_cast<uint32_t *>(row)[w] = lo;
+            } else {
+                if (w < WT - 1) *reinterpret_cast<uint32_t *>(row + e + 4 * w) = __funnelshift_r(lo, tile[r][w + 1], 8 * e);
+                if (w < 4) {
+                    const bool head = static_cast<uint32_t>(w) < e;
+                    const uint32_t word = tile[r][head ? 0 : WT - 1];
+                    row[head ? w : 4 * (WT - 1) + w] = static_cast<unsigned char>(word >> (8 * w));
+                }
+            }
+        }
+        return;
+    }
+    // ragged tiles and unaligned time rows: one output byte per step
+    for (int q = threadIdx.x; q < TC * TU; q += 256) {
+        const int u = q % TU, c = q / TU;
+        const int64_t t = 2 * (u0 + u);
+        if (t >= p.nsamps || c0 + c >= p.nchans) continue;
+        const int sh = ((c0 + c) & 1) * 4;
+        const uint32_t a = in[t * in_pitch + (c0 + c) / 2] >> sh, b = in[(t + 1) * in_pitch + (c0 + c) / 2] >> sh;
+        out[static_cast<int64_t>(c0 + c) * out_pitch + u0 + u] = static_cast<uint8_t>((a & 15u) | (b & 15u) << 4);
+    }
+}
+
 // ------------------------------------------------------------------ fused transpose + interleave
 // Time-major input [nsamps][nchans] straight into the lane-interleaved workspace X (what
 // transpose_kernel + interleave_kernel do in two HBM round trips).  A CTA owns TC = 128 bytes
@@ -1630,6 +1715,11 @@ int launch_bin_time(int mode, const BinParams &p_in, void *stream)
 int launch_transpose(int mode, const TransposeParams &p, void *stream)
 {
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (mode == DD_U4) {
+        const dim3 g4(static_cast<unsigned>((p.nsamps / 2 + 127) / 128), static_cast<unsigned>((p.nchans + 255) / 256));
+        transpose_u4_kernel<<<g4, 256, 0, st>>>(p);
+        return static_cast<int>(cudaGetLastError());
+    }
     const int P = mode == DD_U8 ? 4 : (mode == DD_U16 ? 2 : 1);
     const dim3 grid(static_cast<unsigned>((p.nsamps + 127) / 128),
                     static_cast<unsigned>((p.nchans + 32 * P - 1) / (32 * P)));

@@ -156,7 +156,7 @@ int dd_survey_execute_tm(dd_survey *s, const void *d_in_tm, void *const *d_out, 
         return run_ranges(s, nullptr, d_in_tm, d_out, cuda_stream);
     // binning works on channel-major rows: transpose once (PAPER.md:370 counts it in t_c), then
     // every range -- binned or not -- reads the channel-major copy
-    if (s->in_dtype == DD_U4) return DD_ERR_UNSUPPORTED_PLAN;  // dd_transpose has no packed 4-bit form
+    if (s->in_dtype == DD_U4 && (s->nchans & 1)) return DD_ERR_UNSUPPORTED_PLAN;  // whole bytes per time row
     const size_t need = block_bytes(s->in_dtype, s->nchans, s->nsamps);
     if (need > s->cm_bytes) {
         cudaFree(s->d_cm);

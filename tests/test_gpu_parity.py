@@ -771,3 +771,53 @@ def test_runs_beside_a_tensor_core_gemm(B, oracle):
             run = oracle.dedisperse_u4 if code == B.DD_U4 else oracle.dedisperse
             assert np.array_equal(d_out.cpu().numpy().view(np.uint32), run(x, plan.shift_table(), plan.out_len))
             assert torch.isfinite(c.float()).all()
+
+
+def _pack_channels(x8_tm):
+    """[nsamps][nchans] values 0..15 -> time-major packed rows of nchans/2 bytes, the even channel of a
+    byte in the low nibble (reading R16); layout only."""
+    return np.ascontiguousarray((x8_tm[:, 0::2] | (x8_tm[:, 1::2] << 4)).astype(np.uint8))
+
+
+@pytest.mark.parametrize("shape", [(256, 4096), (512, 1000), (130, 5002), (38, 998), (2, 2), (300, 70002)])
+def test_standalone_transpose_packed_u4(B, shape):
+    """dd_transpose for DD_U4: time-major packed along channels -> channel-major packed along time,
+    against numpy's transpose of the unpacked values (whole tiles, ragged tiles, output rows that do
+    not start on a word)."""
+    import torch
+    nchans, nsamps = shape
+    rng = np.random.default_rng([nchans, nsamps, 4])
+    x8 = rng.integers(0, 16, (nchans, nsamps)).astype(np.uint8)          # [c][t]
+    x_tm = _pack_channels(np.ascontiguousarray(x8.T))                    # [t][c/2]
+    d_out = torch.full((nchans, nsamps // 2), 0xAB, dtype=torch.uint8, device="cuda")
+    B.transpose(torch.from_numpy(x_tm).cuda(), d_out, nchans, nsamps, B.DD_U4)
+    torch.cuda.synchronize()
+    assert np.array_equal(d_out.cpu().numpy(), W.pack_u4(x8))
+    for bad in ((nchans + 1, nsamps), (nchans, nsamps + 1)):
+        with pytest.raises(B.DDError) as e:
+            B.transpose(torch.from_numpy(x_tm).cuda(), d_out, bad[0], bad[1], B.DD_U4)
+        assert e.value.status == B.DD_ERR_INVALID_ARG
+
+
+def test_survey_packed_u4_time_major_with_binning(B, oracle):
+    """A 4-bit survey from a time-major block with binned ranges: packed transpose, dd_bin_time (4-bit
+    -> 8-bit sums), 4-bit and 8-bit plans; against the oracle chain."""
+    import torch
+    nchans, nsamps = 96, 24000
+    ranges = [(0.0, 1.0, 24, 1), (24.0, 2.0, 12, 2), (48.0, 4.0, 8, 4)]
+    rng = np.random.default_rng(9)
+    x8 = rng.integers(0, 16, (nchans, nsamps)).astype(np.uint8)
+    xp = W.pack_u4(x8)
+    x_tm = _pack_channels(np.ascontiguousarray(x8.T))
+    with B.Survey(nchans, nsamps, 1500.0, -2.0, 64e-6, ranges, B.DD_U4) as sv:
+        outs = sv.execute_tm(torch.from_numpy(x_tm).cuda())
+        torch.cuda.synchronize()
+        for (start, step, count, factor), got in zip(ranges, outs):
+            dms = start + np.arange(count) * step
+            otab, omx = oracle.shift_table(nchans, 1500.0, -2.0, 64e-6 * factor, dms)
+            if factor == 1:
+                ref = oracle.dedisperse_u4(xp, otab, nsamps - omx)
+            else:
+                xb = oracle.bin_time(xp, factor, packed_u4=True)          # uint8 sums
+                ref = oracle.dedisperse(xb, otab, xb.shape[1] - omx)
+            assert np.array_equal(got.cpu().numpy().view(np.uint32), ref)
