@@ -821,3 +821,20 @@ def test_survey_packed_u4_time_major_with_binning(B, oracle):
                 xb = oracle.bin_time(xp, factor, packed_u4=True)          # uint8 sums
                 ref = oracle.dedisperse(xb, otab, xb.shape[1] - omx)
             assert np.array_equal(got.cpu().numpy().view(np.uint32), ref)
+
+
+def test_host_timeline_reports_every_chunk(B, oracle):
+    """dd_plan_host_timeline: one entry per chunk of the latest dd_execute_host call, times in order."""
+    rng = np.random.default_rng(3)
+    nchans, nsamps = 64, 40000
+    x = _rand_input(rng, np.uint8, nchans, nsamps)
+    with B.Plan(nchans, nsamps, 1500.0, -2.0, 64e-6, np.arange(16) * 2.0, B.DD_U8) as plan:
+        assert len(plan.host_timeline()[0]) == 0          # no host call yet
+        plan.set_host_chunks(4)
+        h_out = np.zeros((plan.ndm, plan.out_len), dtype=np.uint32)
+        plan.execute_host(x, h_out)
+        assert np.array_equal(h_out, oracle.dedisperse(x, plan.shift_table(), plan.out_len))
+        ob, h2d, pre, main, d2h = plan.host_timeline()
+        assert len(ob) == 4 and ob[0] == 0 and (np.diff(ob) > 0).all()
+        assert (h2d <= pre).all() and (pre <= main).all() and (main <= d2h).all()
+        assert (np.diff(main) >= 0).all() and d2h[-1] > 0
