@@ -481,11 +481,32 @@ static int host_schedule(const dd_plan *plan, int64_t *edge)
         // between a chunk may grow as long as its copy hides behind the previous chunk's kernels.
         // (A finer 12-chunk geometric taper starting at one j tile measured slower -- headline
         // 70.0 ms against 68.7 ms, 4-bit 46.6 against 43.9: every extra launch pays a partial wave.)
-        static const double frac[dd_plan::kHostChunks] = {0.04, 0.07, 0.12, 0.20, 0.25, 0.20, 0.09, 0.03};
+        double frac[dd_plan::kHostChunks] = {0.04, 0.07, 0.12, 0.20, 0.25, 0.20, 0.09, 0.03};
+        int nfrac = dd_plan::kHostChunks;
+#ifdef DD_TUNING
+        // tuning builds only: DD_HOST_TAPER="4,12,28,32,20,4" (per cent, at most kHostChunks entries)
+        if (const char *e = std::getenv("DD_HOST_TAPER")) {
+            int n = 0;
+            double sum = 0.0, v[dd_plan::kHostChunks];
+            const char *q = e;
+            while (*q && n < dd_plan::kHostChunks) {
+                char *end = nullptr;
+                const double x = std::strtod(q, &end);
+                if (end == q || !(x > 0.0) || !std::isfinite(x)) break;
+                v[n++] = x;
+                sum += x;
+                q = *end == ',' ? end + 1 : end;
+            }
+            if (n > 0 && sum > 0.0) {
+                for (int i = 0; i < n; ++i) frac[i] = v[i] / sum;
+                nfrac = n;
+            }
+        }
+#endif
         double cum = 0.0;
-        for (int g = 0; g < dd_plan::kHostChunks; ++g) {
+        for (int g = 0; g < nfrac; ++g) {
             cum += frac[g];
-            int64_t e = g + 1 == dd_plan::kHostChunks
+            int64_t e = g + 1 == nfrac
                             ? plan->out_len
                             : static_cast<int64_t>(cum * static_cast<double>(plan->out_len)) / tile * tile;
             if (e > plan->out_len) e = plan->out_len;
