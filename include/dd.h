@@ -69,7 +69,8 @@ int dd_shift_table_build(int nchans, double f_high_MHz, double chan_bw_MHz, doub
  * DD_ERR_OVERFLOW (u8: 255*nchans >= 2^32; u16: 65535*nchans >= 2^32; u4: 15*nchans >= 2^32); DD_ERR_ALLOC;
  * DD_ERR_CUDA; DD_ERR_UNSUPPORTED_DEVICE; DD_ERR_UNSUPPORTED_PLAN.
  * The library reads no environment variable.  (A tuning build, `build.py --tuning`, adds the A/B
- * kernel shapes of profiles/r02_tuning.md and honours DD_FORCE_VARIANT=<n>; never the default.)
+ * kernel shapes of profiles/r02_tuning.md and honours DD_FORCE_VARIANT=<n>, DD_PANEL=<n> and
+ * DD_HOST_TAPER=<per-cent list>; never the default.)
  */
 int dd_plan_create(dd_plan **out, int nchans, int64_t nsamps, double f_high_MHz,
                    double chan_bw_MHz, double tsamp_s, const double *dm_list, int ndm,
@@ -203,6 +204,17 @@ int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_str
  * fused time-major pre-pass of dd_execute_tm.  Errors as dd_execute_host and dd_execute_tm.
  */
 int dd_execute_host_tm(dd_plan *plan, const void *h_in_tm, void *h_out, void *cuda_stream);
+
+/*
+ * The host-buffer pipeline without the final wait: queues every copy and kernel of dd_execute_host
+ * (time_major == 0) or dd_execute_host_tm (time_major != 0) and returns.  The transform is complete --
+ * h_out fully written, h_in no longer read -- when `cuda_stream` reaches the point of the call (the
+ * call makes that stream wait for the last copy back); both host buffers must stay valid and untouched
+ * until then.  Calls on ONE plan are serialised by that dependency (the plan owns one set of device
+ * buffers); a streaming caller alternates between two plans on two streams, so that the copies of block
+ * n+1 overlap the kernels of block n -- bench.py's `e2e` does exactly that.  Errors as dd_execute_host.
+ */
+int dd_execute_host_async(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream, int time_major);
 
 /*
  * Chunk count of dd_execute_host / dd_execute_host_tm for this plan: 0 = the default schedule

@@ -28,7 +28,7 @@ INFO = {"D_DM": 0, "D_J": 1, "LANES": 2, "L": 3, "SMEM_BYTES": 4, "GRID": 5, "TH
 
 # every symbol include/dd.h declares (tests check the .so exports all of them)
 SYMBOLS = ("dd_shift_table_build", "dd_plan_create", "dd_plan_shift_table", "dd_execute",
-           "dd_execute_host", "dd_execute_host_tm", "dd_execute_tm", "dd_transpose", "dd_bin_time",
+           "dd_execute_host", "dd_execute_host_tm", "dd_execute_host_async", "dd_execute_tm", "dd_transpose", "dd_bin_time",
            "dd_plan_set_host_chunks", "dd_plan_host_timeline", "dd_plan_info", "dd_plan_set_timing", "dd_plan_kernel_times",
            "dd_probe", "dd_plan_destroy", "dd_strerror", "dd_version",
            "dd_survey_create", "dd_survey_num_ranges", "dd_survey_plan", "dd_survey_range_dtype",
@@ -73,6 +73,8 @@ def lib() -> ctypes.CDLL:
         L.dd_execute_host.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p]
         L.dd_execute_host_tm.restype = c.c_int
         L.dd_execute_host_tm.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p]
+        L.dd_execute_host_async.restype = c.c_int
+        L.dd_execute_host_async.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p, c.c_int]
         L.dd_execute_tm.restype = c.c_int
         L.dd_execute_tm.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p]
         L.dd_bin_time.restype = c.c_int
@@ -226,6 +228,14 @@ class Plan:
         rc = lib().dd_execute_host_tm(self._h, _host_ptr(h_in_tm), _host_ptr(h_out), _stream_ptr(stream))
         if rc != DD_OK:
             raise DDError(rc, "dd_execute_host_tm")
+
+    # -- dd_execute_host_async
+    def execute_host_async(self, h_in, h_out, stream=None, time_major: bool = False) -> None:
+        """Queue the host-buffer pipeline and return; complete when `stream` reaches this point."""
+        rc = lib().dd_execute_host_async(self._h, _host_ptr(h_in), _host_ptr(h_out), _stream_ptr(stream),
+                                         1 if time_major else 0)
+        if rc != DD_OK:
+            raise DDError(rc, "dd_execute_host_async")
 
     # -- dd_plan_set_host_chunks
     def set_host_chunks(self, nchunks: int) -> None:

@@ -415,17 +415,23 @@ int dd_plan_kernel_times(dd_plan *plan, int max_n, float *interleave_ms, float *
 // columns travel device->host on a second copy stream.  PCIe is full duplex, so a step costs
 // about max(H2D, kernels, D2H) plus one chunk of fill and drain instead of their sum.  The
 // kernels see a chunk as a smaller block of the same plan (same shift and tiling tables).
-static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream, bool tm);
+static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream, bool tm, bool async);
 
 int dd_execute_host(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream)
 {
-    return execute_host_impl(plan, h_in, h_out, cuda_stream, false);
+    return execute_host_impl(plan, h_in, h_out, cuda_stream, false, false);
 }
 
 int dd_execute_host_tm(dd_plan *plan, const void *h_in_tm, void *h_out, void *cuda_stream)
 {
     if (plan && plan->in_dtype == DD_U4 && (plan->nchans & 1)) return DD_ERR_UNSUPPORTED_PLAN;
-    return execute_host_impl(plan, h_in_tm, h_out, cuda_stream, true);
+    return execute_host_impl(plan, h_in_tm, h_out, cuda_stream, true, false);
+}
+
+int dd_execute_host_async(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream, int time_major)
+{
+    if (plan && time_major && plan->in_dtype == DD_U4 && (plan->nchans & 1)) return DD_ERR_UNSUPPORTED_PLAN;
+    return execute_host_impl(plan, h_in, h_out, cuda_stream, time_major != 0, true);
 }
 
 // Streams and events of the host-buffer path, created on first use: all of them or none.
@@ -539,7 +545,7 @@ int dd_plan_set_host_chunks(dd_plan *plan, int nchunks)
 
 // tm: the host block is time-major [nsamps][nchans]; a chunk's new samples are then ONE contiguous
 // range of it (a plain 1-D copy) and the chunk runs through the fused time-major pre-pass.
-static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream, bool tm)
+static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream, bool tm, bool async)
 {
     if (!plan || !h_in || !h_out) return DD_ERR_INVALID_ARG;
     const dd::Tiling &t = plan->til;
@@ -652,6 +658,10 @@ static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void 
     for (int g = 0; g <= G; ++g) plan->last_edge[g] = edge[g];
     // every main kernel precedes a copy on st_d2h; the caller's stream also waits for the odd chunks
     if (G > 1) cudaStreamWaitEvent(st, plan->ev_done[((G - 1) & 1) ? G - 1 : G - 2], 0);
+    // ... and for the last copy back, so that "the caller's stream has reached this point" means
+    // "h_out is complete" (what the asynchronous form promises)
+    cudaStreamWaitEvent(st, plan->ev_out[G - 1], 0);
+    if (async) return cudaGetLastError() == cudaSuccess ? DD_OK : fail(DD_ERR_CUDA);
     if (cudaStreamSynchronize(plan->st_d2h) != cudaSuccess) return fail(DD_ERR_CUDA);
     if (cudaStreamSynchronize(st) != cudaSuccess) return fail(DD_ERR_CUDA);
     return DD_OK;

@@ -838,3 +838,33 @@ def test_host_timeline_reports_every_chunk(B, oracle):
         assert len(ob) == 4 and ob[0] == 0 and (np.diff(ob) > 0).all()
         assert (h2d <= pre).all() and (pre <= main).all() and (main <= d2h).all()
         assert (np.diff(main) >= 0).all() and d2h[-1] > 0
+
+
+@pytest.mark.parametrize("time_major", [False, True])
+def test_execute_host_async_two_blocks_in_flight(B, oracle, time_major):
+    """dd_execute_host_async: two plans on two streams with different blocks in flight at once, and
+    the same plan called twice in a row (serialised by its stream dependency); results are complete
+    when the streams have been synchronised and equal the oracle's."""
+    import torch
+    rng = np.random.default_rng(12)
+    nchans, nsamps = 96, 50000
+    dms = np.arange(30) * 1.5
+    xs = [_rand_input(rng, np.uint8, nchans, nsamps) for _ in range(3)]
+    hin = [torch.from_numpy(np.ascontiguousarray(x.T if time_major else x)).pin_memory() for x in xs]
+    plans = [B.Plan(nchans, nsamps, 1500.0, -2.0, 64e-6, dms, B.DD_U8) for _ in range(2)]
+    try:
+        for p in plans:
+            p.set_host_chunks(3)
+        houts = [torch.zeros((plans[0].ndm, plans[0].out_len), dtype=torch.int32).pin_memory() for _ in range(3)]
+        streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+        plans[0].execute_host_async(hin[0], houts[0], streams[0], time_major)
+        plans[1].execute_host_async(hin[1], houts[1], streams[1], time_major)
+        plans[0].execute_host_async(hin[2], houts[2], streams[0], time_major)   # same plan again: after block 0
+        for s in streams:
+            s.synchronize()
+        tab = plans[0].shift_table()
+        for x, h in zip(xs, houts):
+            assert np.array_equal(h.numpy().view(np.uint32), oracle.dedisperse(x, tab, plans[0].out_len))
+    finally:
+        for p in plans:
+            p.destroy()
