@@ -212,7 +212,10 @@ int dd_execute_host_tm(dd_plan *plan, const void *h_in_tm, void *h_out, void *cu
  * call makes that stream wait for the last copy back); both host buffers must stay valid and untouched
  * until then.  Calls on ONE plan are serialised by that dependency (the plan owns one set of device
  * buffers); a streaming caller alternates between two plans on two streams, so that the copies of block
- * n+1 overlap the kernels of block n -- bench.py's `e2e` does exactly that.  Errors as dd_execute_host.
+ * n+1 overlap the kernels of block n -- bench.py's `e2e` does exactly that.  Default schedule of this form:
+ * 4 equal chunks (the neighbouring blocks hide the first copy in and the last copy out, so the taper of the
+ * synchronous form is not needed) unless the block's copies take longer than its kernels (then the taper);
+ * dd_plan_set_host_chunks overrides it.  Errors as dd_execute_host.
  */
 int dd_execute_host_async(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream, int time_major);
 

@@ -473,7 +473,7 @@ static int make_host_objects(dd_plan *plan)
 // the number of chunks (1 .. kHostChunks).  Chunk lengths are whole j tiles when the block is
 // long enough, else a multiple of 16 samples per lane (keeps every chunk's rows as aligned as
 // the caller's).
-static int host_schedule(const dd_plan *plan, int64_t *edge)
+static int host_schedule(const dd_plan *plan, int64_t *edge, bool async)
 {
     const dd::Tiling &t = plan->til;
     const int NL = t.shape.lanes();
@@ -481,7 +481,21 @@ static int host_schedule(const dd_plan *plan, int64_t *edge)
     const int64_t unit = static_cast<int64_t>(NL) * 16;
     int G = 0;
     edge[0] = 0;
-    if (plan->host_chunks == 0 && plan->out_len >= 32 * tile) {
+    // The asynchronous form is for callers that keep several blocks in flight: the neighbouring blocks
+    // hide a block's first copy in and last copy out, so a few equal chunks (fewer repeated pre-pass
+    // halos and partial waves) beat the taper: headline 61.4 against 62.8 ms per block, 4-bit 38.2 against
+    // 40.1 (profiles/r02_tuning.md).
+    // Blocks whose copies take longer than their kernels (lowfreq: 8.6 GB in for 126 ms of kernels) keep
+    // the taper in both forms: there the copy engine, not the GPU, must never idle (161 against 166 ms).
+    bool copy_bound = false;
+    {
+        const double adds = static_cast<double>(plan->ndm) * plan->out_len * plan->nchans;
+        const double rate = plan->in_dtype == DD_U4 ? 54e12 : plan->in_dtype == DD_U8 ? 33e12 : plan->in_dtype == DD_U16 ? 17e12 : 9e12;
+        const double in_b = static_cast<double>(plan->nchans) * sample_bytes(plan->in_dtype, plan->nsamps);
+        const double out_b = static_cast<double>(plan->ndm) * plan->out_len * 4.0;
+        copy_bound = (in_b > out_b ? in_b : out_b) / 50e9 > 0.9 * adds / rate;
+    }
+    if (plan->host_chunks == 0 && (!async || copy_bound) && plan->out_len >= 32 * tile) {
         // Tapered schedule: only the first chunk's host->device copy (chunk + max_shift halo) and
         // the last chunk's device->host copy are exposed, so those two chunks are small; in
         // between a chunk may grow as long as its copy hides behind the previous chunk's kernels.
@@ -520,7 +534,7 @@ static int host_schedule(const dd_plan *plan, int64_t *edge)
         }
         return G;
     }
-    int want = plan->host_chunks ? plan->host_chunks : 6;
+    int want = plan->host_chunks ? plan->host_chunks : (async ? 4 : 6);
     if (!plan->host_chunks) {  // at least 8 j tiles per chunk so that the grid still fills the GPU
         const int64_t by_tiles = plan->out_len / (8 * tile);
         if (want > by_tiles) want = static_cast<int>(by_tiles);
@@ -565,7 +579,7 @@ static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void 
     if (const int rc = make_host_objects(plan); rc != DD_OK) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     int64_t edge[dd_plan::kHostChunks + 1];  // chunk g = output samples [edge[g], edge[g+1])
-    const int G = host_schedule(plan, edge);
+    const int G = host_schedule(plan, edge, async);
 
     const unsigned char *hin = static_cast<const unsigned char *>(h_in);
     unsigned char *din = static_cast<unsigned char *>(plan->d_in_own);
