@@ -230,7 +230,8 @@ int dd_plan_set_host_chunks(dd_plan *plan, int nchunks);
  * account of the end-to-end time: for chunk g (up to max_chunks of them) the first output sample
  * out_begin[g] and the times, in milliseconds after the call started on `cuda_stream`, at which its
  * input had arrived on the device (h2d_ms), its pre-pass (pre_ms) and main kernel (main_ms) had
- * finished and its output had arrived on the host (d2h_ms).  Any array may be NULL.  Returns the number
+ * finished and its output had arrived on the host (d2h_ms); waits for that call to finish if it was an
+ * asynchronous one.  Any array may be NULL.  Returns the number
  * of chunks written (0 if the plan has not run a host call), or a negative dd_status.
  */
 int dd_plan_host_timeline(dd_plan *plan, int max_chunks, int64_t *out_begin, float *h2d_ms, float *pre_ms,

@@ -689,6 +689,11 @@ int dd_plan_host_timeline(dd_plan *plan, int max_chunks, int64_t *out_begin, flo
     const int G = plan->last_chunks < max_chunks ? plan->last_chunks : max_chunks;
     // ev_done[last_chunks] was recorded on the caller's stream when the call started
     const cudaEvent_t t0 = plan->ev_done[plan->last_chunks];
+    // (an asynchronous call may still be running: wait for its last copy back)
+    if (cudaEventSynchronize(plan->ev_out[plan->last_chunks - 1]) != cudaSuccess) {
+        cudaGetLastError();
+        return DD_ERR_CUDA;
+    }
     for (int g = 0; g < G; ++g) {
         float a = 0.f, b = 0.f, c = 0.f, d = 0.f;
         if (cudaEventElapsedTime(&a, t0, plan->ev_in[g]) != cudaSuccess ||
