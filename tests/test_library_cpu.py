@@ -148,3 +148,21 @@ def test_header_is_plain_c(tmp_path):
     res = subprocess.run([gcc, "-std=c99", "-Wall", "-Wextra", "-Werror", "-pedantic", "-I", inc, "-c",
                           str(src), "-o", str(tmp_path / "use_dd.o")], capture_output=True, text=True)
     assert res.returncode == 0, res.stderr
+
+
+def test_survey_create_rejects_bad_ranges_without_a_gpu():
+    """dd_survey_create validates its ranges before it touches the device."""
+    import ctypes
+    from paper_2311_05341_b200 import binding as B
+    L = B.lib()
+    h = ctypes.c_void_p(1)
+    rng = (B._DmRange * 1)(B._DmRange(0.0, 1.0, 10, 3))          # 3 is not a binning factor
+    assert L.dd_survey_create(ctypes.byref(h), 8, 1000, 1500.0, -1.0, 64e-6, ctypes.cast(rng, ctypes.c_void_p), 1, B.DD_U8) == B.DD_ERR_INVALID_ARG
+    assert h.value is None
+    rng = (B._DmRange * 1)(B._DmRange(0.0, 1.0, 0, 1))           # no trials
+    assert L.dd_survey_create(ctypes.byref(h), 8, 1000, 1500.0, -1.0, 64e-6, ctypes.cast(rng, ctypes.c_void_p), 1, B.DD_U8) == B.DD_ERR_INVALID_ARG
+    rng = (B._DmRange * 1)(B._DmRange(0.0, 1.0, 5, 2))           # 16-bit samples cannot be binned
+    assert L.dd_survey_create(ctypes.byref(h), 8, 1000, 1500.0, -1.0, 64e-6, ctypes.cast(rng, ctypes.c_void_p), 1, B.DD_U16) == B.DD_ERR_UNSUPPORTED_PLAN
+    assert L.dd_survey_create(ctypes.byref(h), 8, 1000, 1500.0, -1.0, 64e-6, None, 0, B.DD_U8) == B.DD_ERR_INVALID_ARG
+    assert L.dd_survey_num_ranges(None) == B.DD_ERR_INVALID_ARG and L.dd_survey_plan(None, 0) is None
+    L.dd_survey_destroy(None)
