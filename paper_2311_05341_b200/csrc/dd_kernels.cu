@@ -14,8 +14,15 @@
 //             W - 256*O at the flush, after at most 256 channels (256*255 < 2^16), into four
 //             uint32 accumulators per word that live in tensor memory (lane-private scratch);
 //        u16: W += w, H += w >> 16; low lane recovered as W - 65536*H at the end;
+//        u4 : eight 4-bit lanes per word stay packed in shared memory (0.5 B per add): W += w
+//             (carries run across nibble lanes), A += odd nibbles of w as byte lanes (LOP3 + LEA.HI);
+//             per stage the byte lanes fold into 16-bit lanes, every <= 4096 channels into uint32
+//             accumulators in tensor memory;
 //        f32: FADD.
-// Also here: transpose_kernel (dd_transpose), bin_time_*_kernel (dd_bin_time).
+//      The grid is rasterised in DM-block panels so that a wave's input footprint is streamed
+//      from HBM once (tile_of_cta).
+// Also here: interleave_u4_kernel / interleave_tm_u4_kernel (4-bit pre-passes), transpose_kernel and
+// transpose_u4_kernel (dd_transpose), bin_time_*_kernel (dd_bin_time).
 // The tensor cores' MMA units are not used: a shifted-diagonal sum is not a contraction.
 #include <cuda_runtime.h>
 
