@@ -41,7 +41,8 @@ typedef enum dd_status {
     DD_ERR_ALLOC = -4,              /* host or device allocation failed */
     DD_ERR_CUDA = -5,               /* a CUDA runtime call or kernel launch failed */
     DD_ERR_UNSUPPORTED_DEVICE = -6, /* current device is not sm_100 (B200) */
-    DD_ERR_UNSUPPORTED_PLAN = -7    /* a single DM trial's staged window exceeds shared memory */
+    DD_ERR_UNSUPPORTED_PLAN = -7,   /* a single DM trial's staged window exceeds shared memory */
+    DD_ERR_STATIC_LIMIT = -8        /* dd_execute_noalloc: ndm*nchans exceeds DD_NOALLOC_MAX_TABLE */
 } dd_status;
 
 /*
@@ -177,6 +178,38 @@ int dd_survey_range_dtype(const dd_survey *survey, int range);
 int dd_survey_execute(dd_survey *survey, const void *d_in, void *const *d_out, void *cuda_stream);
 int dd_survey_execute_tm(dd_survey *survey, const void *d_in_tm, void *const *d_out, void *cuda_stream);
 void dd_survey_destroy(dd_survey *survey);
+
+/*
+ * The transform (Eq. 3) without any device allocation, for small problems.
+ *
+ * Everything else in this header needs a plan, and dd_plan_create calls cudaMalloc.  Some callers cannot:
+ * a process whose own pool already holds all of the card's memory (cudaMalloc fails there), or a real-time
+ * stage that may not stall its neighbours (cudaMalloc / cudaFree synchronise the whole device).  This call
+ * is for them.  It allocates nothing on the device or the host and calls no routine that does: its single
+ * piece of scratch, the device copy of the shift table, is a fixed array of DD_NOALLOC_MAX_TABLE int32
+ * entries (4 MiB) built into libdd.so -- every GPU that loads the library carries those 4 MiB until the
+ * process exits, whether or not this call is ever made.
+ *   table : HOST, int32 [ndm][nchans] row-major, every entry >= 0 -- what dd_shift_table_build writes into
+ *           a buffer of the caller's; read before the call returns.
+ *   d_in  : DEVICE, dense [nchans][nsamps] of in_dtype (DD_U8 / DD_U16 / DD_F32 / DD_U4, layouts as dd_execute).
+ *   d_out : DEVICE, dense [ndm][out_len], out_len = nsamps - max(table); uint32, or float32 for DD_F32
+ *           (channels summed in ascending order).  Every element is overwritten.
+ * Runs on the CURRENT device, asynchronously on `cuda_stream`: one copy of the table into the built-in
+ * array, then one kernel that reads each sample from global memory (no shared-memory tiling: expect a
+ * few per cent of dd_execute's rate -- with a plan available, use the plan).
+ * The first call on each device also looks up the array's device address (cudaGetSymbolAddress; nothing
+ * is allocated).  Make that first call ahead of any stream capture.
+ * All calls on a device share the one array, and it keeps the previous call's table: each call rewrites
+ * the ndm*nchans entries it reads, so no clearing is needed, but two calls whose GPU work can overlap
+ * (different streams, no ordering between them) race on it and give wrong sums.  Calls on one stream are safe.
+ * Errors: DD_ERR_INVALID_ARG (nulls, sizes, dtype, a negative entry, odd nsamps for DD_U4);
+ * DD_ERR_STATIC_LIMIT (ndm*nchans > DD_NOALLOC_MAX_TABLE -- nothing is launched);
+ * DD_ERR_SHIFT_TOO_LARGE (max(table) >= nsamps); DD_ERR_OVERFLOW (DD_U16 with 65535*nchans >= 2^32);
+ * DD_ERR_UNSUPPORTED_DEVICE (not sm_100); DD_ERR_CUDA.
+ */
+#define DD_NOALLOC_MAX_TABLE (1 << 20)
+int dd_execute_noalloc(const int32_t *table, int ndm, int nchans, int64_t nsamps, int in_dtype,
+                       const void *d_in, void *d_out, void *cuda_stream);
 
 /*
  * The same transform with HOST buffers: h_in [nchans][nsamps], h_out [ndm][out_len].

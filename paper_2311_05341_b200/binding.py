@@ -22,12 +22,15 @@ DD_ERR_ALLOC = -4
 DD_ERR_CUDA = -5
 DD_ERR_UNSUPPORTED_DEVICE = -6
 DD_ERR_UNSUPPORTED_PLAN = -7
+DD_ERR_STATIC_LIMIT = -8
+NOALLOC_MAX_TABLE = 1 << 20   # DD_NOALLOC_MAX_TABLE
 
 INFO = {"D_DM": 0, "D_J": 1, "LANES": 2, "L": 3, "SMEM_BYTES": 4, "GRID": 5, "THREADS": 6,
         "WORKSPACE_BYTES": 7, "STAGE_BYTES": 8, "LAUNCHES": 9, "CH": 10, "NSTAGE": 11, "PANEL": 12}
 
 # every symbol include/dd.h declares (tests check the .so exports all of them)
 SYMBOLS = ("dd_shift_table_build", "dd_plan_create", "dd_plan_shift_table", "dd_execute",
+           "dd_execute_noalloc",
            "dd_execute_host", "dd_execute_host_tm", "dd_execute_host_async", "dd_execute_tm", "dd_transpose", "dd_bin_time",
            "dd_plan_set_host_chunks", "dd_plan_host_timeline", "dd_plan_info", "dd_plan_set_timing", "dd_plan_kernel_times",
            "dd_probe", "dd_plan_destroy", "dd_strerror", "dd_version",
@@ -69,6 +72,9 @@ def lib() -> ctypes.CDLL:
                                           c.POINTER(c.c_int64), c.POINTER(c.c_int32)]
         L.dd_execute.restype = c.c_int
         L.dd_execute.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p]
+        L.dd_execute_noalloc.restype = c.c_int
+        L.dd_execute_noalloc.argtypes = [c.c_void_p, c.c_int, c.c_int, c.c_int64, c.c_int, c.c_void_p, c.c_void_p,
+                                         c.c_void_p]
         L.dd_execute_host.restype = c.c_int
         L.dd_execute_host.argtypes = [c.c_void_p, c.c_void_p, c.c_void_p, c.c_void_p]
         L.dd_execute_host_tm.restype = c.c_int
@@ -166,6 +172,20 @@ def bin_time(d_in, d_out, nchans: int, nsamps: int, factor: int, in_dtype: int, 
                            int(in_dtype), _stream_ptr(stream))
     if rc != DD_OK:
         raise DDError(rc, "dd_bin_time")
+
+
+def execute_noalloc(table, nsamps: int, in_dtype: int, d_in, d_out, stream=None) -> None:
+    """dd_execute_noalloc: the transform for a caller that may not allocate device memory (its pool owns
+    the card, or it cannot afford cudaMalloc's device-wide stall).  ``table``: host int32 [ndm, nchans]
+    from dd_shift_table_build, at most NOALLOC_MAX_TABLE entries; d_in / d_out: device tensors the caller
+    already owns.  Calls that can overlap on the GPU race on the library's built-in table array."""
+    tab = np.ascontiguousarray(table, dtype=np.int32)
+    if tab.ndim != 2:
+        raise ValueError("table must be [ndm, nchans]")
+    rc = lib().dd_execute_noalloc(tab.ctypes.data, int(tab.shape[0]), int(tab.shape[1]), int(nsamps),
+                                  int(in_dtype), _dev_ptr(d_in), _dev_ptr(d_out), _stream_ptr(stream))
+    if rc != DD_OK:
+        raise DDError(rc, "dd_execute_noalloc")
 
 
 class Plan:

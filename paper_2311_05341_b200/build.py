@@ -18,7 +18,7 @@ _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(_ROOT, "include")
 LIB = os.path.join(_HERE, "libdd.so")
-SOURCES = ["dd_host.cpp", "dd_kernels.cu", "dd_api.cu", "dd_survey.cu", "dd_probe.cu"]
+SOURCES = ["dd_host.cpp", "dd_kernels.cu", "dd_api.cu", "dd_survey.cu", "dd_probe.cu", "dd_noalloc.cu"]
 HEADERS = [os.path.join(CSRC, "dd_internal.h"), os.path.join(INCLUDE, "dd.h")]
 
 NVCC_FLAGS = [

@@ -752,6 +752,7 @@ const char *dd_strerror(int status)
     case DD_ERR_CUDA: return "CUDA runtime error";
     case DD_ERR_UNSUPPORTED_DEVICE: return "current device is not sm_100";
     case DD_ERR_UNSUPPORTED_PLAN: return "staged window of one DM trial exceeds shared memory";
+    case DD_ERR_STATIC_LIMIT: return "shift table larger than DD_NOALLOC_MAX_TABLE entries (dd_execute_noalloc's built-in scratch)";
     default: return "unknown status";
     }
 }
