@@ -94,7 +94,9 @@ int dd_plan_shift_table(const dd_plan *plan, const int32_t **table, int64_t *out
  *   cuda_stream: a cudaStream_t (NULL = the legacy default stream).
  * Asynchronous on that stream: no allocation, no synchronisation, no host read of the data.
  * The plan's workspace is used by the call, so executions of ONE plan must be ordered on
- * one stream (or otherwise serialised by the caller); different plans are independent.
+ * one stream (or otherwise serialised by the caller); different plans are independent.  (One case is
+ * handled for you: a dd_execute queued while a dd_execute_host_async of the same plan is pending waits
+ * for that call's last copy back, whichever stream it was given.)
  * Errors: DD_ERR_INVALID_ARG (null plan / pointers), DD_ERR_CUDA (launch failure).
  */
 int dd_execute(const dd_plan *plan, const void *d_in, void *d_out, void *cuda_stream);
@@ -243,8 +245,10 @@ int dd_execute_host_tm(dd_plan *plan, const void *h_in_tm, void *h_out, void *cu
  * (time_major == 0) or dd_execute_host_tm (time_major != 0) and returns.  The transform is complete --
  * h_out fully written, h_in no longer read -- when `cuda_stream` reaches the point of the call (the
  * call makes that stream wait for the last copy back); both host buffers must stay valid and untouched
- * until then.  Calls on ONE plan are serialised by that dependency (the plan owns one set of device
- * buffers); a streaming caller alternates between two plans on two streams, so that the copies of block
+ * until then.  Host-buffer calls on ONE plan are serialised whatever streams they are queued from: each
+ * waits for the previous one's last copy back (the plan owns one set of device buffers), and so does a
+ * dd_execute / dd_execute_tm that follows a host call.  The reverse is the caller's to order: a host call
+ * after a dd_execute that is still running on ANOTHER stream.  A streaming caller alternates between two plans on two streams, so that the copies of block
  * n+1 overlap the kernels of block n -- bench.py's `e2e` does exactly that.  Default schedule of this form:
  * 4 equal chunks (the neighbouring blocks hide the first copy in and the last copy out, so the taper of the
  * synchronous form is not needed) unless the block's copies take longer than its kernels (then the taper);

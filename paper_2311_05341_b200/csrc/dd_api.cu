@@ -299,10 +299,21 @@ int launch_main(const dd_plan *plan, const BlockGeom &g, const uint32_t *X, void
                                                                                                 : DD_OK;
 }
 
+// A host-buffer call of this plan (dd_execute_host*, possibly asynchronous and queued from another
+// stream) owns the plan's workspaces and device buffers until its last copy back has finished:
+// ev_out[last_chunks - 1] marks that moment.  Whatever uses them next waits for it first.  A no-op
+// for plans that never took the host path (nothing is queued, no event exists yet).
+void wait_for_pending_host_call(const dd_plan *plan, cudaStream_t st)
+{
+    if (plan->host_made && plan->last_chunks > 0)
+        cudaStreamWaitEvent(st, plan->ev_out[plan->last_chunks - 1], 0);
+}
+
 int launch_block(const dd_plan *plan, const BlockGeom &g, const void *d_in, int64_t in_pitch,
                  void *d_out, int64_t out_pitch, cudaStream_t st, const cudaEvent_t *ev,
                  bool time_major = false)
 {
+    wait_for_pending_host_call(plan, st);
     if (ev) cudaEventRecord(ev[0], st);
     int rc = launch_prepass(plan, g, d_in, in_pitch, plan->d_X, st, time_major);
     if (rc != DD_OK) return rc;
@@ -618,6 +629,11 @@ static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void 
         cudaGetLastError();
         return rc;
     };
+    // An earlier host call of this plan may still be running, queued from ANOTHER stream (two
+    // asynchronous calls, or a streaming caller that changed streams): it owns d_in_own, d_X / d_X2
+    // and d_out_own until its last copy back.  `st` waits for that; every other stream of this call
+    // starts behind ev_done[G] below, so the whole call does.
+    wait_for_pending_host_call(plan, st);
     // the plan's streams start after whatever the caller has queued on `st`
     if (cudaEventRecord(plan->ev_done[G], st) != cudaSuccess) return DD_ERR_CUDA;
     cudaStreamWaitEvent(plan->st_h2d, plan->ev_done[G], 0);

@@ -203,6 +203,19 @@ def test_unsorted_and_repeated_dm_list(B, oracle):
     check_against_oracle(oracle, x, out, otab, out_len)
 
 
+def test_rasterisation_panel_does_not_depend_on_dm_order(B):
+    """The panel size (a DRAM-traffic heuristic, never a correctness matter) is taken from the shift span
+    between the smallest and the largest DM, wherever they sit in dm_list: a descending list plans the
+    same panel as the ascending one (round-2 advice: it used rows 0 and ndm-1 and fell back to one panel)."""
+    dms = np.arange(480) * 0.5
+    panels = []
+    for order in (dms, dms[::-1].copy()):
+        with B.Plan(2048, 60000, 1500.0, -300.0 / 2048, 64e-6, order, B.DD_U8) as plan:
+            panels.append(plan.info("PANEL"))
+            ndb = -(-plan.ndm // plan.info("D_DM"))
+    assert panels[0] == panels[1] and 1 <= panels[0] < ndb   # more than one panel, so the order could matter
+
+
 def test_single_impulse_response(B):
     # a single 1 at (c*, tau) in zeros -> out[d][tau - s(d,c*)] = 1 and 0 elsewhere
     nchans, nsamps, cstar, tau = 40, 3000, 29, 1777
@@ -868,3 +881,34 @@ def test_execute_host_async_two_blocks_in_flight(B, oracle, time_major):
     finally:
         for p in plans:
             p.destroy()
+
+
+def test_one_plan_host_calls_from_different_streams_are_serialised(B, oracle):
+    """One plan, host calls queued from DIFFERENT streams with nothing ordering them, then a dd_execute
+    on a third: the plan owns one set of device buffers, so each call must wait for the previous host
+    call's last copy back (round-2 advice: before, the second call's copies in could overwrite the
+    first call's input while its kernels were still reading it).  A long first block makes the overlap
+    window wide; every plane must equal the oracle's."""
+    import torch
+    rng = np.random.default_rng(77)
+    nchans, nsamps = 256, 400000
+    dms = np.arange(96) * 1.0
+    xs = [_rand_input(rng, np.uint8, nchans, nsamps) for _ in range(3)]
+    hin = [torch.from_numpy(x).pin_memory() for x in xs]
+    with B.Plan(nchans, nsamps, 1500.0, -1.0, 64e-6, dms, B.DD_U8) as plan:
+        houts = [torch.zeros((plan.ndm, plan.out_len), dtype=torch.int32).pin_memory() for _ in range(2)]
+        d_in = torch.from_numpy(xs[2]).cuda()
+        d_out = torch.zeros((plan.ndm, plan.out_len), dtype=torch.int32, device="cuda")
+        s = [torch.cuda.Stream() for _ in range(3)]
+        torch.cuda.synchronize()
+        for rep in range(2):
+            plan.execute_host_async(hin[0], houts[0], s[0])
+            plan.execute_host_async(hin[1], houts[1], s[1])   # another stream, nothing orders it after s[0]
+            plan.execute(d_in, d_out, s[2])                   # device path while both are pending
+            torch.cuda.synchronize()
+            tab = plan.shift_table()
+            for x, got in ((xs[0], houts[0].numpy()), (xs[1], houts[1].numpy()), (xs[2], d_out.cpu().numpy())):
+                assert np.array_equal(got.view(np.uint32), oracle.dedisperse(x, tab, plan.out_len)), rep
+            for h in houts:
+                h.zero_()
+            d_out.zero_()
