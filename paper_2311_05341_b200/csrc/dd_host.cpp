@@ -149,9 +149,19 @@ bool build_tiling(const KernelShape &shape, int variant, const int32_t *table, i
     // lowfreq 8 where the model says 12, headline 15-22 for 18, c3 16 for 16), so 0.7 of it is
     // taken; panels are made equal.
     {
+        // s(d,c) grows with the DM in every channel, so the rows of the largest and the smallest DM
+        // bound every column; the last channel (lowest frequency, largest coefficient) tells which
+        // rows those are -- dm_list need not be ascending
+        int d_lo = 0, d_hi = 0;
+        for (int d = 1; d < ndm; ++d) {
+            const int32_t s = table[static_cast<size_t>(d) * nchans + (nchans - 1)];
+            if (s < table[static_cast<size_t>(d_lo) * nchans + (nchans - 1)]) d_lo = d;
+            if (s >= table[static_cast<size_t>(d_hi) * nchans + (nchans - 1)]) d_hi = d;  // ascending list: rows 0 and ndm-1
+        }
         double span = 0.0;
         for (int c = 0; c < nchans; ++c)
-            span += static_cast<double>(table[static_cast<size_t>(ndm - 1) * nchans + c] - table[c]);
+            span += static_cast<double>(table[static_cast<size_t>(d_hi) * nchans + c] -
+                                        table[static_cast<size_t>(d_lo) * nchans + c]);
         span = span * S / t->ndb;
         const double tile = static_cast<double>(t->nch_pad) * D_J * S;
         double nb = span > 0.0 ? 0.7 * std::sqrt(static_cast<double>(num_sms) * tile / span) : t->ndb;
