@@ -15,9 +15,12 @@ collective; value = units of all ranks / max-over-ranks time ("scaling": "weak")
 --impl reference: the CPU oracle (oracle/dedisp_oracle.c), as it stands, timed on the host
 cores on a bounded sample of the same workload (a subset of DM rows per step).
 
-Besides the contract's keys the line carries: `e2e` (dd_execute_host, pinned host buffers, copies
-inside the timed region), `roofline` (shared-memory pipe, the binding one) with `roofline_alu` and
-`roofline_hbm`, `cpu_baseline` (the oracle on the host cores, about 10 s), `kernels_ms`,
+Besides the contract's keys the line carries: `e2e` (dd_execute_host_async, pinned host buffers, copies
+inside the timed region), `roofline` (shared-memory pipe, for every input type; peak at the SM clock
+sampled during the timed region, `frac_at_probe_clock` beside it) with `roofline_alu`, `roofline_hbm`
+and, for 4-bit input, `roofline_alu_pipe`; `configs` (default headline run at N = 1 only: c2, c3,
+lowfreq, headline_u4, paper52, largeshift and survey52, device-resident, each with its own clocks and
+roofline; --no-configs leaves it out); `cpu_baseline` (the oracle on the host cores, about 10 s), `kernels_ms`,
 `realtime_factor` (Eq. 10), `time_major` (dd_execute_tm / dd_execute_host_tm / dd_transpose) and
 `time_binning` (dd_bin_time).  Extra workloads: headline_u4 (packed 4-bit), paper52 (the paper's
 section 5.2 plan), survey52 (a multi-range binned plan over a time-major block through
@@ -85,13 +88,22 @@ class ClockSampler:
             self.rows.append((time.perf_counter(), line.strip()))
 
     def stop(self, t0: float, t1: float):
+        res = self.window(t0, t1)
+        self.close()
+        return res
+
+    def close(self):
+        if self.proc is not None:
+            self.proc.terminate()
+
+    def window(self, t0: float, t1: float):
+        """Clocks and throttle reasons of the samples taken in [t0, t1] (the sampler keeps running)."""
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         time.sleep(0.15)
-        self.proc.terminate()
         sm, mx, reasons = [], None, set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for ts, line in self.rows:
+        for ts, line in list(self.rows):
             if not (t0 <= ts <= t1 + 0.12):
                 continue
             f = [x.strip() for x in line.split(",")]
@@ -258,9 +270,13 @@ PROBE_UNITS = {"SM_COUNT": "SMs", "SM_CLOCK_MHZ": "MHz", "LDS32": "B/clk/SM", "L
                "F32_ADDS_TMEM_4_OF_8_NO_FILL": "f32 adds/clk/SM"}
 
 
-def measure_peaks(B):
-    """Every dd_probe key -> value (lane-instructions or bytes per clock per SM, SM clock, SM count)."""
-    return {k: B.probe(k) for k in B.PROBES}
+ROOFLINE_PROBES = ("SM_COUNT", "SM_CLOCK_MHZ", "LDS32", "LDS64", "LDS128", "IADD3", "FADD")
+
+
+def measure_peaks(B, keys=None):
+    """dd_probe key -> value (lane-instructions or bytes per clock per SM, SM clock, SM count); every key
+    for --probe-peaks, only the roofline denominators (ROOFLINE_PROBES) inside a benchmark run."""
+    return {k: B.probe(k) for k in (keys or B.PROBES)}
 
 
 def run_probe_peaks(args):
@@ -282,6 +298,156 @@ def run_probe_peaks(args):
             "fp32_add_peak_tlane_s": p["FADD"] * nsm * mhz * 1e6 / 1e12}
     print(json.dumps(line))
     return 0
+
+
+def _sources_sha16():
+    """First 16 hex digits of the sha256 of the sources that decide the main kernel's DRAM traffic (the
+    kernels and the plan-time tiling / rasterisation): a traffic capture is quoted only for the tree it
+    was taken on (the GPU box has no .git to ask)."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in ("dd_kernels.cu", "dd_host.cpp"):
+        with open(os.path.join(ROOT, "paper_2311_05341_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+TRAFFIC_CSV = os.path.join("profiles", "r03_traffic.csv")
+
+
+def _traffic_for(name: str):
+    """(DRAM bytes per dedisperse_kernel launch, note) from the committed ncu capture of this workload,
+    or (None, why) when there is none for the current sources."""
+    path = os.path.join(ROOT, TRAFFIC_CSV)
+    if not os.path.exists(path):
+        return None, "no " + TRAFFIC_CSV
+    sha = _sources_sha16()
+    with open(path) as f:
+        rows = [ln.split(",") for ln in f.read().splitlines()[1:] if ln and not ln.startswith("#")]
+    for fld in rows:
+        if fld[0] == name:
+            if fld[-1].strip() != sha:
+                return None, ("%s holds a capture of other kernel sources (%s, now %s): not quoted"
+                              % (TRAFFIC_CSV, fld[-1].strip(), sha))
+            return int(fld[1]), ("ncu dram__bytes_read.sum + dram__bytes_write.sum of one launch, %s, "
+                                 "sources sha16 %s" % (TRAFFIC_CSV, sha))
+    return None, "no row for %s in %s" % (name, TRAFFIC_CSV)
+
+
+def _smem_roofline(name, adds, in_b, hbm_alg_bytes, main_s, share, probed, run_mhz, overridden=False):
+    """The main kernel against the shared-memory pipe (one sample read from shared memory per add,
+    DESIGN.md section 7).  The peak is dd_probe's measured bytes per clock per SM times the SM clock
+    SAMPLED DURING THE TIMED REGION (the probes themselves run cooler and clock a little lower); the
+    fraction at the probe's own clock is printed beside it."""
+    n_sm = int(probed["SM_COUNT"])
+    b_clk = max(probed["LDS32"], probed["LDS64"], probed["LDS128"])
+    probe_mhz = probed["SM_CLOCK_MHZ"]
+    mhz = run_mhz if run_mhz else probe_mhz
+    peak = n_sm * b_clk * mhz * 1e6 / 1e9
+    ach = adds * in_b / main_s / 1e9
+    traffic, tnote = (None, "shape overridden on the command line") if overridden else _traffic_for(name)
+    return {"bound": "smem", "kernel": "dedisperse_kernel", "achieved": ach, "peak": peak, "unit": "GB/s",
+            "frac": ach / peak, "peak_clock_mhz": mhz,
+            "peak_clock": "clocks.sm_mhz of this timed region" if run_mhz else "dd_probe clock (no nvidia-smi sample)",
+            "frac_at_probe_clock": ach / (n_sm * b_clk * probe_mhz * 1e6 / 1e9),
+            "peak_kind": "measured (dd_probe) %.1f B/clk/SM x %d SMs x %.0f MHz; paper Eq. 8 form: 128 B/clk/SM"
+                         % (b_clk, n_sm, mhz),
+            "traffic": traffic, "traffic_note": tnote, "algorithmic_hbm_bytes": hbm_alg_bytes,
+            "hbm_waste": (traffic / hbm_alg_bytes) if traffic else None,
+            "algorithmic_bytes_per_add": in_b, "adds_per_launch": adds,
+            "kernel_ms": main_s * 1e3, "share_of_step": share}
+
+
+def _time_config(B, name, sampler, probed, min_region_s=0.6):
+    """One extra workload for the default line's `configs` block: device-resident step time (CUDA
+    events, >= 5 timed steps after 2 warm-ups, at least `min_region_s` of timed work so that nvidia-smi
+    sees it), adds/s, the main kernel's shared-memory roofline and the real-time factor."""
+    import torch
+    cfg = W.ALL_CONFIGS[name]
+    plan = B.Plan(cfg.nchans, cfg.nsamps, cfg.f_high, cfg.chan_bw, cfg.tsamp, cfg.dm_list, cfg.in_dtype)
+    try:
+        table = plan.shift_table() if cfg.npulses else None
+        x = W.make_input_torch(cfg, "cuda", table, plan.out_len)
+        del table
+        odt = torch.float32 if cfg.in_dtype == W.F32 else torch.int32
+        out = torch.empty((plan.ndm, plan.out_len), dtype=odt, device="cuda")
+        adds = plan.ndm * plan.out_len * cfg.nchans
+        stream = torch.cuda.current_stream()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        plan.execute(x, out)
+        e0.record(stream)
+        plan.execute(x, out)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        steps = int(min(64, max(5, np.ceil(min_region_s * 1e3 / max(e0.elapsed_time(e1), 1e-3)))))
+        plan.set_timing(True)
+        t0 = time.perf_counter()
+        e0.record(stream)
+        for _ in range(steps):
+            plan.execute(x, out)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        ms_step = e0.elapsed_time(e1) / steps
+        plan.set_timing(False)
+        il_ms, main_ms = plan.kernel_times(steps)
+        clocks = sampler.window(t0, t1)
+        main_s, il_s = float(np.mean(main_ms)) * 1e-3, float(np.mean(il_ms)) * 1e-3
+        in_b = W.ELEM_BYTES[cfg.in_dtype]
+        hbm_alg = int(cfg.nchans * cfg.nsamps * in_b) + plan.ndm * plan.out_len * 4
+        return {"value": adds / (ms_step * 1e-3), "unit": UNIT, "ms_per_step": ms_step, "steps": steps, "warmup": 2,
+                "in_dtype": W.DTYPE_NAME[cfg.in_dtype], "nchans": cfg.nchans, "nsamps": cfg.nsamps, "ndm": cfg.ndm,
+                "dm_step": cfg.dm_step, "out_len": plan.out_len, "adds_per_step": adds, "tile": _tile_string(plan),
+                "kernels_ms": {"interleave_kernel": il_s * 1e3, "dedisperse_kernel": main_s * 1e3},
+                "roofline": _smem_roofline(name, adds, in_b, hbm_alg, main_s, main_s / (main_s + il_s), probed,
+                                           clocks.get("sm_mhz")),
+                "realtime_factor": cfg.nsamps * cfg.tsamp / (ms_step * 1e-3), "clocks": clocks,
+                "gpu_launches": steps * plan.info("LAUNCHES")}
+    finally:
+        plan.destroy()
+
+
+def _time_survey(B, name, sampler, min_region_s=0.6):
+    """A survey workload for the `configs` block: dd_survey_execute_tm over a resident time-major block
+    (transpose + time binning + every range), the paper's pipeline real-time factor (Eq. 10)."""
+    import torch
+    sc = W.SURVEYS[name]
+    gen = W.Config(sc.name, sc.nchans, sc.nsamps, sc.in_dtype, sc.f_high, sc.chan_bw, sc.tsamp, 1, 0.0,
+                   seed=sc.seed, mean=sc.mean, sd=sc.sd)
+    x_tm = W.noise_torch(gen, "cuda").t().contiguous()
+    sv = B.Survey(sc.nchans, sc.nsamps, sc.f_high, sc.chan_bw, sc.tsamp, sc.ranges, sc.in_dtype)
+    try:
+        adds = sum(n * ol * sc.nchans for n, ol in zip(sv.ndm, sv.out_len))
+        stream = torch.cuda.current_stream()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        sv.execute_tm(x_tm)
+        e0.record(stream)
+        sv.execute_tm(x_tm)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        steps = int(min(32, max(5, np.ceil(min_region_s * 1e3 / max(e0.elapsed_time(e1), 1e-3)))))
+        t0 = time.perf_counter()
+        e0.record(stream)
+        for _ in range(steps):
+            sv.execute_tm(x_tm)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        ms_step = e0.elapsed_time(e1) / steps
+        nbin = len({r[3] for r in sc.ranges if r[3] > 1})
+        return {"value": adds / (ms_step * 1e-3), "unit": UNIT, "ms_per_step": ms_step, "steps": steps, "warmup": 2,
+                "api": "dd_survey_execute_tm (transpose + time binning + dedispersion of every range)",
+                "layout": "time-major", "nchans": sc.nchans, "nsamps": sc.nsamps,
+                "ranges": [list(r) for r in sc.ranges], "adds_per_step": adds,
+                "realtime_factor": {"R_eq10": sc.t_obs / (ms_step * 1e-3), "t_obs_s": sc.t_obs, "t_c_ms": ms_step},
+                "clocks": sampler.window(t0, t1),
+                "gpu_launches": steps * ((1 if nbin else 0) + nbin + 2 * len(sc.ranges))}
+    finally:
+        sv.destroy()
+
+
+EXTRA_LINE_CONFIGS = ("c2", "c3", "lowfreq", "headline_u4", "paper52", "largeshift")
+EXTRA_LINE_SURVEYS = ("survey52",)
 
 
 # ------------------------------------------------------------------------- our arm
@@ -309,7 +475,7 @@ def run_ours(args):
 
     cfg = W.ALL_CONFIGS[args.config]
     hbm_gbs, sm_max_mhz, peak_kind = _peaks()
-    probed = measure_peaks(B) if rank == 0 else None   # before the timed region: a second of GPU time
+    probed = measure_peaks(B, ROOFLINE_PROBES) if rank == 0 else None   # before the timed region
     plan = B.Plan(cfg.nchans, cfg.nsamps, cfg.f_high, cfg.chan_bw, cfg.tsamp, cfg.dm_list, cfg.in_dtype)
     table = plan.shift_table() if cfg.npulses else None
     # every rank: its own block (seed offset by rank), resident in HBM before timing starts
@@ -350,6 +516,25 @@ def run_ours(args):
     # whole job = sum of units over ranks / max of time over ranks (no data-path collective)
     value, ms_total = shard.job_throughput(float(adds) * args.steps, ms_total, dist, "cuda")
     ms_step = ms_total / args.steps
+
+    if args.quick:
+        # profiler captures (ncu -k regex:dedisperse ...): the device-resident region only, said in the line
+        if rank == 0:
+            line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                    "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+                    "vs_baseline": None, "dtype": _dtype_name(cfg), "data": "synthetic",
+                    "config": _config_dict(cfg, plan), "tile": _tile_string(plan),
+                    "kernels_ms": {"interleave_kernel": float(np.mean(il_ms)), "dedisperse_kernel": float(np.mean(main_ms))},
+                    "quick": "device-resident region only: no e2e, roofline, cpu_baseline or configs (--quick)",
+                    "gpu_launches": args.steps * plan.info("LAUNCHES"), "clocks": clocks}
+            sys.stdout.flush()
+            os.dup2(saved_stdout, 1)
+            print(json.dumps(line), flush=True)
+        plan.destroy()
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
+        return 0
 
     # ---- end to end through the C ABI with HOST buffers (H2D + kernels + D2H in the timed region)
     # A streaming caller keeps two blocks in flight: dd_execute_host_async on two plans and two streams,
@@ -496,60 +681,38 @@ def run_ours(args):
     # from shared memory (best of LDS.32/.64/.128), IADD3 lane-instructions per clock per SM, and
     # the SM clock during the probes; the derived figures (paper Eq. 8) are reported beside them
     n_sm = int(probed["SM_COUNT"])
-    clk = probed["SM_CLOCK_MHZ"] * 1e6
-    smem_b_clk = max(probed["LDS32"], probed["LDS64"], probed["LDS128"])
-    int_peak = n_sm * probed["IADD3"] * clk
-    smem_peak_gbs = n_sm * smem_b_clk * clk / 1e9
-    smem_peak_derived = N_SM * SMEM_BYTES_PER_SM_CLK * sm_max_mhz * 1e6 / 1e9
     int_peak_derived = N_SM * INT_LANES_PER_SM_CLK * sm_max_mhz * 1e6
-    in_b = W.ELEM_BYTES[cfg.in_dtype]
-    smem_b = in_b                                       # bytes a sample occupies in shared memory (4-bit: 0.5)
-    smem_alg_bytes = adds * smem_b                      # one sample read from shared memory per add
+    in_b = W.ELEM_BYTES[cfg.in_dtype]                   # bytes a sample occupies in shared memory (4-bit: 0.5)
     hbm_alg_bytes = int(cfg.nchans * cfg.nsamps * in_b) + plan.ndm * plan.out_len * 4
-    traffic = None
-    # DRAM bytes (read + write) of one dedisperse_kernel launch from the committed ncu captures of
-    # this kernel (profiles/r02_traffic.csv names the capture; profiles/r02_summary.md the commit)
-    tpath = os.path.join(ROOT, "profiles", "r02_traffic.csv")
     overridden = (cfg.nsamps, cfg.ndm, cfg.dm_step) != W.ALL_CONFIGS_SHAPE.get(cfg.name)
-    if os.path.exists(tpath) and not overridden:
-        with open(tpath) as f:
-            for ln in f.read().splitlines()[1:]:
-                fld = ln.split(",")
-                if fld[0] == cfg.name:
-                    traffic = int(fld[1])
     share = main_s / (main_s + il_s)
-    # The dominant kernel reads one sample from shared memory per add: its binding roofline is the
-    # shared-memory pipe (ncu: 90-99 % of peak wavefronts), reported in bytes.
-    roofline = {"bound": "smem", "kernel": "dedisperse_kernel",
-                "achieved": smem_alg_bytes / main_s / 1e9, "peak": smem_peak_gbs, "unit": "GB/s",
-                "frac": smem_alg_bytes / main_s / 1e9 / smem_peak_gbs, "traffic": traffic,
-                "traffic_note": "DRAM bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r02_traffic.csv, r02_summary.md); algorithmic HBM bytes %d"
-                                % hbm_alg_bytes,
-                "peak_kind": "measured (dd_probe): %.1f B/clk/SM x %d SMs x %.0f MHz; derived (paper Eq. 8) %.0f GB/s"
-                             % (smem_b_clk, n_sm, probed["SM_CLOCK_MHZ"], smem_peak_derived),
-                "algorithmic_bytes_per_add": smem_b, "adds_per_launch": adds,
-                "kernel_ms": main_s * 1e3, "share_of_step": share}
+    run_mhz = clocks.get("sm_mhz") if clocks else None
+    # The dominant kernel reads one sample from shared memory per add: `roofline` is the shared-memory
+    # pipe for EVERY input type (the paper's own accounting, Eq. 8; ncu: 90-99 % of peak wavefronts for
+    # u8 / u16 / f32), reported in bytes, with the peak at the clock sampled during the timed region.
+    roofline = _smem_roofline(cfg.name, adds, in_b, hbm_alg_bytes, main_s, share, probed, run_mhz, overridden)
+    alu_mhz = run_mhz if run_mhz else probed["SM_CLOCK_MHZ"]
+    int_peak = n_sm * probed["IADD3"] * alu_mhz * 1e6
     roofline_alu = {"bound": "alu", "achieved": kadds / 1e12, "peak": int_peak / 1e12, "unit": "Tadd/s",
                     "frac": kadds / int_peak,
                     "peak_kind": "measured (dd_probe): %.1f IADD3 lanes/clk/SM x %d SMs x %.0f MHz; derived %.2f Tadd/s"
-                                 % (probed["IADD3"], n_sm, probed["SM_CLOCK_MHZ"], int_peak_derived / 1e12),
+                                 % (probed["IADD3"], n_sm, alu_mhz, int_peak_derived / 1e12),
                     "note": "sample-adds against one-add-per-lane integer peak (BASELINE.json's metric); "
                             "a packed add performs 8 (u4) / 4 (u8) / 2 (u16) sample-adds, so frac may exceed 1"}
+    roofline_alu_pipe = None
     if cfg.in_dtype == W.U4:
-        # The 4-bit kernel is bound by the alu pipe, not by shared memory (ncu:
-        # alu 83 % busy, shared-memory wavefronts 76 %): per 32-bit word (8 sample-adds) the odd
-        # nibbles cost one LOP3 and one LEA.HI there, which no formulation found avoids.  The
-        # shared-memory view is kept beside it.
+        # Secondary view for the 4-bit kernel, which sits nearer its alu-pipe limit than its shared-memory
+        # one (ncu, profiles/r02_headline_u4_dedisperse_details.txt: alu 83 % busy,
+        # shared-memory wavefronts 76 %): per 32-bit word (8 sample-adds) the odd nibbles cost one LOP3 and
+        # one LEA.HI on that pipe.  A builder-defined instruction count, so not comparable across types:
+        # it explains the shared-memory fraction above, it does not replace it.
         alu_ops = adds * 2.0 / 8.0
-        roofline_smem = roofline
-        roofline = {"bound": "alu", "kernel": "dedisperse_kernel", "achieved": alu_ops / main_s / 1e12,
-                    "peak": int_peak / 1e12, "unit": "T lane-instructions/s",
-                    "frac": alu_ops / main_s / int_peak, "traffic": traffic,
-                    "traffic_note": roofline_smem["traffic_note"],
-                    "peak_kind": "measured (dd_probe): %.1f alu-pipe lanes/clk/SM x %d SMs x %.0f MHz"
-                                 % (probed["IADD3"], n_sm, probed["SM_CLOCK_MHZ"]),
-                    "algorithmic_alu_instructions_per_add": 0.25, "adds_per_launch": adds,
-                    "kernel_ms": main_s * 1e3, "share_of_step": share, "smem_view": roofline_smem}
+        roofline_alu_pipe = {"bound": "alu", "kernel": "dedisperse_kernel", "achieved": alu_ops / main_s / 1e12,
+                             "peak": int_peak / 1e12, "unit": "T lane-instructions/s",
+                             "frac": alu_ops / main_s / int_peak,
+                             "algorithmic_alu_instructions_per_add": 0.25,
+                             "note": "alu-pipe lane-instructions (LOP3 + LEA.HI per 8 adds) against the measured "
+                                     "IADD3 issue rate; secondary to `roofline`"}
     roofline_hbm = {"bound": "hbm", "achieved": hbm_alg_bytes / (ms_step * 1e-3) / 1e9, "peak": hbm_gbs,
                     "unit": "GB/s", "frac": hbm_alg_bytes / (ms_step * 1e-3) / 1e9 / hbm_gbs,
                     "peak_kind": peak_kind + " copy bandwidth",
@@ -558,15 +721,41 @@ def run_ours(args):
     x_host = h_in.numpy() if cfg.in_dtype != W.U16 else h_in.view(torch.int16).numpy().view(np.uint16)
     cpu_base, _ = time_oracle(cfg, 1, 1, x=x_host)
     cpu_tiled = time_tiled(cfg, x_host)
+    gpu_launches = args.steps * plan.info("LAUNCHES")
+    tile_string, config_dict = _tile_string(plan), _config_dict(cfg, plan)
+    realtime = {"t_obs_over_t": cfg.nsamps * cfg.tsamp / (ms_step * 1e-3),
+                "out_len_tsamp_over_t": plan.out_len * cfg.tsamp / (ms_step * 1e-3)}
+    # ---- the other workloads, device-resident, in the same line (default run of the headline at N = 1):
+    # BASELINE.json's other configs and the section 8(f) workloads, each with its own clocks and roofline
+    configs = None
+    if cfg.name == "headline" and not overridden and world == 1 and not args.no_configs:
+        plan.destroy()
+        del x, out, h_in, x_host, h_out
+        torch.cuda.empty_cache()
+        configs = {}
+        sampler2 = ClockSampler(local_rank)
+        sampler2.start()
+        time.sleep(0.3)
+        t_cfg0 = time.perf_counter()
+        for name in EXTRA_LINE_CONFIGS:
+            configs[name] = _time_config(B, name, sampler2, probed)
+            torch.cuda.empty_cache()
+        for name in EXTRA_LINE_SURVEYS:
+            configs[name] = _time_survey(B, name, sampler2)
+            torch.cuda.empty_cache()
+        sampler2.close()
+        configs["_note"] = ("device-resident dd_execute (surveys: dd_survey_execute_tm) per workload, CUDA events, "
+                            ">= 5 timed steps after 2 warm-ups, clocks sampled per workload; %.0f s in all; "
+                            "their launches are not in the line's gpu_launches" % (time.perf_counter() - t_cfg0))
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": _dtype_name(cfg),
-            "data": "synthetic", "config": _config_dict(cfg, plan), "tile": _tile_string(plan),
-            "realtime_factor": {"t_obs_over_t": cfg.nsamps * cfg.tsamp / (ms_step * 1e-3),
-                                "out_len_tsamp_over_t": plan.out_len * cfg.tsamp / (ms_step * 1e-3)},
+            "data": "synthetic", "config": config_dict, "tile": tile_string,
+            "realtime_factor": realtime,
             "value_nominal": world * cfg.ndm * cfg.nsamps * cfg.nchans / (ms_step * 1e-3),
             "kernels_ms": {"interleave_kernel": il_s * 1e3, "dedisperse_kernel": main_s * 1e3},
-            "roofline": roofline, "roofline_alu": roofline_alu, "roofline_hbm": roofline_hbm,
+            "roofline": roofline, "roofline_alu": roofline_alu, "roofline_alu_pipe": roofline_alu_pipe,
+            "roofline_hbm": roofline_hbm,
             "measured_peaks": probed,
             "cpu_baseline": cpu_base, "cpu_baseline_tiled": cpu_tiled,
             "time_major": tm, "time_binning": binning,
@@ -577,8 +766,8 @@ def run_ours(args):
                     "single_call_ms": ms_single,
                     "single_call_note": "dd_execute_host alone (synchronous, one block in flight); its timeline below",
                     "e2e_verified": e2e_verified, "timeline": e2e_timeline},
-            "gpu_launches": args.steps * plan.info("LAUNCHES"),
-            "clocks": clocks}
+            "gpu_launches": gpu_launches,
+            "clocks": clocks, "configs": configs}
     sys.stdout.flush()
     os.dup2(saved_stdout, 1)
     print(json.dumps(line), flush=True)
@@ -771,11 +960,15 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--probe-peaks", action="store_true",
                     help="only run the library's on-chip peak probes (dd_probe) and print them")
+    ap.add_argument("--no-configs", action="store_true",
+                    help="headline only: leave out the `configs` block (the other workloads, about a minute)")
+    ap.add_argument("--quick", action="store_true",
+                    help="device-resident region only (for profiler captures); the line says so")
     ap.add_argument("--nsamps", type=int, default=0,
                     help="override the config's block length (sanity check: adds/s should not depend "
                          "on the observation length, PAPER.md:287); the line's config says so")
     ap.add_argument("--dm-step", type=float, default=0.0,
-                    help="override the config's DM step (walks down the DM-block ladder: profiles/r02_ladder.md)")
+                    help="override the config's DM step (walks down the DM-block ladder: the ladder table in profiles/r02_summary.md)")
     ap.add_argument("--ndm", type=int, default=0, help="override the config's number of DM trials")
     args = ap.parse_args()
     _apply_overrides(args)
