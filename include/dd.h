@@ -69,9 +69,9 @@ int dd_shift_table_build(int nchans, double f_high_MHz, double chan_bw_MHz, doub
  * nsamps <= 0, unknown dtype); DD_ERR_SHIFT_TOO_LARGE (max shift >= nsamps);
  * DD_ERR_OVERFLOW (u8: 255*nchans >= 2^32; u16: 65535*nchans >= 2^32; u4: 15*nchans >= 2^32); DD_ERR_ALLOC;
  * DD_ERR_CUDA; DD_ERR_UNSUPPORTED_DEVICE; DD_ERR_UNSUPPORTED_PLAN.
- * The library reads no environment variable.  (A tuning build, `build.py --tuning`, adds the A/B
- * kernel shapes of profiles/r02_tuning.md and honours DD_FORCE_VARIANT=<n>, DD_PANEL=<n> and
- * DD_HOST_TAPER=<per-cent list>; never the default.)
+ * The library reads no environment variable.  (A tuning build, `build.py --tuning`, is a separate
+ * file, libdd_tuning.so: it adds the A/B kernel shapes of profiles/r02_tuning.md and honours
+ * DD_FORCE_VARIANT=<n>, DD_PANEL=<n> and DD_HOST_TAPER=<per-cent list>; libdd.so never does.)
  */
 int dd_plan_create(dd_plan **out, int nchans, int64_t nsamps, double f_high_MHz,
                    double chan_bw_MHz, double tsamp_s, const double *dm_list, int ndm,
@@ -97,7 +97,11 @@ int dd_plan_shift_table(const dd_plan *plan, const int32_t **table, int64_t *out
  * one stream (or otherwise serialised by the caller); different plans are independent.  (One case is
  * handled for you: a dd_execute queued while a dd_execute_host_async of the same plan is pending waits
  * for that call's last copy back, whichever stream it was given.)
- * Errors: DD_ERR_INVALID_ARG (null plan / pointers), DD_ERR_CUDA (launch failure).
+ * The plan belongs to the device that was current at dd_plan_create: call with that device current
+ * (an in-process multi-GPU caller does cudaSetDevice first); from another device every dd_execute* and
+ * dd_survey_execute* returns DD_ERR_INVALID_ARG and launches nothing.  dd_transpose, dd_bin_time and
+ * dd_execute_noalloc take no plan and run on the current device.
+ * Errors: DD_ERR_INVALID_ARG (null plan / pointers, wrong current device), DD_ERR_CUDA (launch failure).
  */
 int dd_execute(const dd_plan *plan, const void *d_in, void *d_out, void *cuda_stream);
 
@@ -251,8 +255,12 @@ int dd_execute_host_tm(dd_plan *plan, const void *h_in_tm, void *h_out, void *cu
  * after a dd_execute that is still running on ANOTHER stream.  A streaming caller alternates between two plans on two streams, so that the copies of block
  * n+1 overlap the kernels of block n -- bench.py's `e2e` does exactly that.  Default schedule of this form:
  * 4 equal chunks (the neighbouring blocks hide the first copy in and the last copy out, so the taper of the
- * synchronous form is not needed) unless the block's copies take longer than its kernels (then the taper);
- * dd_plan_set_host_chunks overrides it.  Errors as dd_execute_host.
+ * synchronous form is not needed) unless the block's copies take longer than its kernels (then the taper).
+ * That comparison is an estimate from the rates of the machine the library was tuned on (a B200 behind a
+ * 50 GB/s-per-direction host link; 54 / 33 / 17 / 9 T adds/s for 4-bit / 8-bit / 16-bit / float32 input): it
+ * chooses between two correct schedules, never affects results, dd_plan_set_host_chunks overrides it and
+ * dd_plan_info(DD_INFO_HOST_CHUNKS / DD_INFO_HOST_TAPER) tells which one the latest call took.
+ * Errors as dd_execute_host.
  */
 int dd_execute_host_async(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream, int time_major);
 
@@ -291,7 +299,9 @@ enum {
     DD_INFO_LAUNCHES = 9,      /* kernels dd_execute launches */
     DD_INFO_CH = 10,           /* channels per pipeline stage */
     DD_INFO_NSTAGE = 11,       /* pipeline stages */
-    DD_INFO_PANEL = 12         /* DM blocks per rasterisation panel of the main kernel's grid */
+    DD_INFO_PANEL = 12,        /* DM blocks per rasterisation panel of the main kernel's grid */
+    DD_INFO_HOST_CHUNKS = 13,  /* time chunks of the latest dd_execute_host* call of this plan (0: none yet) */
+    DD_INFO_HOST_TAPER = 14    /* 1 if that call took the tapered schedule, 0 if equal chunks */
 };
 int64_t dd_plan_info(const dd_plan *plan, int what);
 
@@ -321,13 +331,8 @@ int dd_plan_kernel_times(dd_plan *plan, int max_n, float *interleave_ms, float *
  *                                IMAD = 32-bit multiply-add, fma pipe; SHIFT_ADD = acc + (x >> k),
  *                                SASS LEA.HI; IMAD_HI = high half multiply-add; IDP4A = 4-way byte dot
  *                                product; LOP3, PRMT, SHF, FADD as named)
- *   DD_PROBE_TMEM_LD             tensor-memory bytes read per clock per SM (tcgen05.ld.32x32b.x8)
- *   DD_PROBE_TMEM_LD_WITH_LDS    the same while the CTA also reads as many bytes with LDS.64
- *   DD_PROBE_F32_ADDS_*          float32 sample-adds per clock per SM of the accumulate loop a
- *                                "tensor memory as a second operand store" kernel would run (DESIGN.md
- *                                section 10), global-memory side left out: every operand from shared memory
- *                                (SMEM_ONLY, the present kernel's loop), or 4 / 8 of every 8 channels copied
- *                                into tensor-memory windows first and read from there (TMEM_4_OF_8; _NO_FILL: windows filled once only)
+ * (A tuning build, libdd_tuning.so, compiled with -DDD_TUNING, has five more keys: the tensor-memory
+ * experiments of DESIGN.md section 10, whose numbers are kept in profiles/r02_peaks.md.)
  * Blocking (synchronises the device); allocates and frees a few MB.  Errors: DD_ERR_INVALID_ARG,
  * DD_ERR_UNSUPPORTED_DEVICE, DD_ERR_ALLOC, DD_ERR_CUDA.
  */
@@ -346,12 +351,19 @@ enum {
     DD_PROBE_SHIFT_ADD = 11,
     DD_PROBE_IMAD_HI = 12,
     DD_PROBE_IDP4A = 13,
-    DD_PROBE_SHF = 14,
+    DD_PROBE_SHF = 14
+#ifdef DD_TUNING
+    /* tensor-memory bytes per clock per SM (tcgen05.ld.32x32b.x8), alone and beside as many LDS.64 bytes;
+     * float32 sample-adds per clock per SM of the accumulate loop of a "tensor memory as a second operand
+     * store" kernel: operands from shared memory only, or 4 of every 8 channels through tensor-memory
+     * windows (refilled / filled once) */
+    ,
     DD_PROBE_TMEM_LD = 15,
     DD_PROBE_TMEM_LD_WITH_LDS = 16,
     DD_PROBE_F32_ADDS_SMEM_ONLY = 17,
     DD_PROBE_F32_ADDS_TMEM_4_OF_8 = 18,
     DD_PROBE_F32_ADDS_TMEM_4_OF_8_NO_FILL = 19
+#endif
 };
 int dd_probe(int what, double *value);
 

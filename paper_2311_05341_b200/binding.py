@@ -26,7 +26,8 @@ DD_ERR_STATIC_LIMIT = -8
 NOALLOC_MAX_TABLE = 1 << 20   # DD_NOALLOC_MAX_TABLE
 
 INFO = {"D_DM": 0, "D_J": 1, "LANES": 2, "L": 3, "SMEM_BYTES": 4, "GRID": 5, "THREADS": 6,
-        "WORKSPACE_BYTES": 7, "STAGE_BYTES": 8, "LAUNCHES": 9, "CH": 10, "NSTAGE": 11, "PANEL": 12}
+        "WORKSPACE_BYTES": 7, "STAGE_BYTES": 8, "LAUNCHES": 9, "CH": 10, "NSTAGE": 11, "PANEL": 12,
+        "HOST_CHUNKS": 13, "HOST_TAPER": 14}
 
 # every symbol include/dd.h declares (tests check the .so exports all of them)
 SYMBOLS = ("dd_shift_table_build", "dd_plan_create", "dd_plan_shift_table", "dd_execute",
@@ -40,10 +41,21 @@ SYMBOLS = ("dd_shift_table_build", "dd_plan_create", "dd_plan_shift_table", "dd_
 # dd_probe keys (include/dd.h DD_PROBE_*)
 PROBES = {"SM_COUNT": 0, "SM_CLOCK_MHZ": 1, "LDS32": 2, "LDS64": 3, "LDS128": 4, "IADD3": 5,
           "VIADD16X2": 6, "IMAD": 7, "FADD": 8, "LOP3": 9, "PRMT": 10, "SHIFT_ADD": 11, "IMAD_HI": 12,
-          "IDP4A": 13, "SHF": 14, "TMEM_LD": 15, "TMEM_LD_WITH_LDS": 16, "F32_ADDS_SMEM_ONLY": 17,
-          "F32_ADDS_TMEM_4_OF_8": 18, "F32_ADDS_TMEM_4_OF_8_NO_FILL": 19}
+          "IDP4A": 13, "SHF": 14}
+# libdd_tuning.so only (use_tuning_library): the tensor-memory experiments of DESIGN.md section 10
+TUNING_PROBES = {"TMEM_LD": 15, "TMEM_LD_WITH_LDS": 16, "F32_ADDS_SMEM_ONLY": 17,
+                 "F32_ADDS_TMEM_4_OF_8": 18, "F32_ADDS_TMEM_4_OF_8_NO_FILL": 19}
 
 _lib = None
+
+
+def use_tuning_library() -> None:
+    """Load libdd_tuning.so (build.py --tuning: extra A/B kernel shapes, DD_FORCE_VARIANT / DD_PANEL /
+    DD_HOST_TAPER) instead of libdd.so in this process.  Call before anything else in this module."""
+    global LIB_PATH
+    if _lib is not None:
+        raise RuntimeError("libdd.so is already loaded; call use_tuning_library() first")
+    LIB_PATH = os.path.join(_HERE, "libdd_tuning.so")
 
 
 class DDError(RuntimeError):
@@ -57,8 +69,9 @@ def lib() -> ctypes.CDLL:
     global _lib
     if _lib is None:
         if not os.path.exists(LIB_PATH):
-            raise ImportError("libdd.so is not built: run `python -m paper_2311_05341_b200.build` "
-                              "(there is no CPU fallback)")
+            raise ImportError("%s is not built: run `python -m paper_2311_05341_b200.build%s` "
+                              "(there is no CPU fallback)"
+                              % (os.path.basename(LIB_PATH), " --tuning" if "tuning" in LIB_PATH else ""))
         L = ctypes.CDLL(LIB_PATH)
         c = ctypes
         L.dd_shift_table_build.restype = c.c_int
@@ -135,7 +148,7 @@ def version() -> str:
 def probe(what: str) -> float:
     """dd_probe: one measured on-chip peak of the current device (keys of PROBES)."""
     v = ctypes.c_double(0.0)
-    rc = lib().dd_probe(PROBES[what], ctypes.byref(v))
+    rc = lib().dd_probe(PROBES[what] if what in PROBES else TUNING_PROBES[what], ctypes.byref(v))
     if rc != DD_OK:
         raise DDError(rc, "dd_probe(%s)" % what)
     return float(v.value)

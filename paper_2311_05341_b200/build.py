@@ -2,8 +2,10 @@
 
     python -m paper_2311_05341_b200.build [--force] [--verbose] [--tuning]
 
---tuning adds -DDD_TUNING: the A/B kernel shapes of profiles/r02_tuning.md and the
-DD_FORCE_VARIANT environment variable exist only in such a build (never the default).
+--tuning adds -DDD_TUNING and writes a SEPARATE library, libdd_tuning.so: the A/B kernel shapes of
+profiles/r02_tuning.md and the DD_FORCE_VARIANT / DD_PANEL / DD_HOST_TAPER environment variables exist
+only there.  libdd.so is never a tuning build; binding.use_tuning_library() (before the first call into
+the library) makes a process load the tuning one instead.
 
 The .so is git-ignored and travels to the GPU box with the gpurun snapshot.
 """
@@ -18,6 +20,7 @@ _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(_ROOT, "include")
 LIB = os.path.join(_HERE, "libdd.so")
+LIB_TUNING = os.path.join(_HERE, "libdd_tuning.so")
 SOURCES = ["dd_host.cpp", "dd_kernels.cu", "dd_api.cu", "dd_survey.cu", "dd_probe.cu", "dd_noalloc.cu"]
 HEADERS = [os.path.join(CSRC, "dd_internal.h"), os.path.join(INCLUDE, "dd.h")]
 
@@ -37,18 +40,19 @@ def _nvcc() -> str:
     return "nvcc"
 
 
-def needs_build() -> bool:
-    if not os.path.exists(LIB):
+def needs_build(lib: str = LIB) -> bool:
+    if not os.path.exists(lib):
         return True
-    t = os.path.getmtime(LIB)
+    t = os.path.getmtime(lib)
     deps = [os.path.join(CSRC, s) for s in SOURCES] + HEADERS + [os.path.abspath(__file__)]
     return any(os.path.getmtime(d) > t for d in deps)
 
 
 def build(force: bool = False, verbose: bool = False, tuning: bool = False) -> str:
-    if not force and not tuning and not needs_build():
-        return LIB
-    tmp = LIB + ".tmp.%d" % os.getpid()
+    lib = LIB_TUNING if tuning else LIB
+    if not force and not needs_build(lib):
+        return lib
+    tmp = lib + ".tmp.%d" % os.getpid()
     cmd = [_nvcc()] + NVCC_FLAGS + ["-I", INCLUDE, "-I", CSRC]
     if tuning:
         cmd += ["-DDD_TUNING"]
@@ -62,8 +66,8 @@ def build(force: bool = False, verbose: bool = False, tuning: bool = False) -> s
         if os.path.exists(tmp):
             os.remove(tmp)
         raise RuntimeError("nvcc failed (exit %d): %s" % (res.returncode, " ".join(cmd)))
-    os.replace(tmp, LIB)
-    return LIB
+    os.replace(tmp, lib)
+    return lib
 
 
 if __name__ == "__main__":

@@ -32,6 +32,7 @@ struct dd_plan {
     cudaEvent_t ev_in[kHostChunks + 1] = {}, ev_done[kHostChunks + 1] = {}, ev_pre[kHostChunks + 1] = {};
     cudaEvent_t ev_out[kHostChunks + 1] = {};  // chunk g's device->host copy has finished
     int last_chunks = 0;             // chunks of the latest dd_execute_host[_tm] call
+    int last_taper = 0;              // 1 if that call took the tapered schedule
     int64_t last_edge[kHostChunks + 1] = {};
     uint32_t *d_X2 = nullptr;  // second chunk workspace: chunk g+1 is interleaved while chunk g is dedispersed
     size_t x2_bytes = 0;
@@ -299,6 +300,15 @@ int launch_main(const dd_plan *plan, const BlockGeom &g, const uint32_t *X, void
                                                                                                 : DD_OK;
 }
 
+// A plan's buffers, streams and events live on the device that was current at dd_plan_create; a launch
+// from another current device would hand that device pointers it cannot use.  One process per GPU never
+// gets here; an in-process multi-GPU caller must cudaSetDevice to the plan's device first.
+bool on_plan_device(const dd_plan *plan)
+{
+    int cur = -1;
+    return cudaGetDevice(&cur) == cudaSuccess && cur == plan->device;
+}
+
 // A host-buffer call of this plan (dd_execute_host*, possibly asynchronous and queued from another
 // stream) owns the plan's workspaces and device buffers until its last copy back has finished:
 // ev_out[last_chunks - 1] marks that moment.  Whatever uses them next waits for it first.  A no-op
@@ -331,6 +341,7 @@ extern "C" {
 int dd_execute(const dd_plan *plan, const void *d_in, void *d_out, void *cuda_stream)
 {
     if (!plan || !d_in || !d_out) return DD_ERR_INVALID_ARG;
+    if (!on_plan_device(plan)) return DD_ERR_INVALID_ARG;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const cudaEvent_t *ev = plan->timing ? plan->ev[plan->timed_count % dd_plan::kRing] : nullptr;
     const BlockGeom g = geom_for(plan, plan->out_len, plan->nsamps);
@@ -343,6 +354,7 @@ int dd_execute_tm(const dd_plan *plan, const void *d_in_tm, void *d_out, void *c
 {
     if (!plan || !d_in_tm || !d_out) return DD_ERR_INVALID_ARG;
     if (plan->in_dtype == DD_U4 && (plan->nchans & 1)) return DD_ERR_UNSUPPORTED_PLAN;  // whole bytes per time row
+    if (!on_plan_device(plan)) return DD_ERR_INVALID_ARG;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const cudaEvent_t *ev = plan->timing ? plan->ev[plan->timed_count % dd_plan::kRing] : nullptr;
     const BlockGeom g = geom_for(plan, plan->out_len, plan->nsamps);
@@ -484,8 +496,9 @@ static int make_host_objects(dd_plan *plan)
 // the number of chunks (1 .. kHostChunks).  Chunk lengths are whole j tiles when the block is
 // long enough, else a multiple of 16 samples per lane (keeps every chunk's rows as aligned as
 // the caller's).
-static int host_schedule(const dd_plan *plan, int64_t *edge, bool async)
+static int host_schedule(const dd_plan *plan, int64_t *edge, bool async, int *tapered)
 {
+    *tapered = 0;
     const dd::Tiling &t = plan->til;
     const int NL = t.shape.lanes();
     const int64_t tile = static_cast<int64_t>(NL) * t.shape.D_J();
@@ -498,6 +511,11 @@ static int host_schedule(const dd_plan *plan, int64_t *edge, bool async)
     // 40.1 (profiles/r02_tuning.md).
     // Blocks whose copies take longer than their kernels (lowfreq: 8.6 GB in for 126 ms of kernels) keep
     // the taper in both forms: there the copy engine, not the GPU, must never idle (161 against 166 ms).
+    // The estimate below uses the rates measured on the B200 this library was tuned on (first-rung kernels:
+    // 54 / 33 / 17 / 9 T adds/s for 4-bit / 8-bit / 16-bit / float32 input) and 50 GB/s per direction for the
+    // host link (PCIe 5 x16 as measured).  It only picks between two correct schedules; on another link or
+    // for a plan on a lower ladder rung dd_plan_set_host_chunks overrides it, and dd_plan_info
+    // (DD_INFO_HOST_CHUNKS / DD_INFO_HOST_TAPER) reports what the latest call took.
     bool copy_bound = false;
     {
         const double adds = static_cast<double>(plan->ndm) * plan->out_len * plan->nchans;
@@ -543,6 +561,7 @@ static int host_schedule(const dd_plan *plan, int64_t *edge, bool async)
             if (e > plan->out_len) e = plan->out_len;
             if (e > edge[G]) edge[++G] = e;
         }
+        *tapered = 1;
         return G;
     }
     int want = plan->host_chunks ? plan->host_chunks : (async ? 4 : 6);
@@ -573,6 +592,7 @@ int dd_plan_set_host_chunks(dd_plan *plan, int nchunks)
 static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void *cuda_stream, bool tm, bool async)
 {
     if (!plan || !h_in || !h_out) return DD_ERR_INVALID_ARG;
+    if (!on_plan_device(plan)) return DD_ERR_INVALID_ARG;
     const dd::Tiling &t = plan->til;
     const int dt = plan->in_dtype;
     const size_t in_bytes = static_cast<size_t>(plan->nchans) * sample_bytes(dt, plan->nsamps);
@@ -590,7 +610,8 @@ static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void 
     if (const int rc = make_host_objects(plan); rc != DD_OK) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     int64_t edge[dd_plan::kHostChunks + 1];  // chunk g = output samples [edge[g], edge[g+1])
-    const int G = host_schedule(plan, edge, async);
+    int tapered = 0;
+    const int G = host_schedule(plan, edge, async, &tapered);
 
     const unsigned char *hin = static_cast<const unsigned char *>(h_in);
     unsigned char *din = static_cast<unsigned char *>(plan->d_in_own);
@@ -685,6 +706,7 @@ static int execute_host_impl(dd_plan *plan, const void *h_in, void *h_out, void 
         cudaEventRecord(plan->ev_out[g], plan->st_d2h);
     }
     plan->last_chunks = G;
+    plan->last_taper = tapered;
     for (int g = 0; g <= G; ++g) plan->last_edge[g] = edge[g];
     // every main kernel precedes a copy on st_d2h; the caller's stream also waits for the odd chunks
     if (G > 1) cudaStreamWaitEvent(st, plan->ev_done[((G - 1) & 1) ? G - 1 : G - 2], 0);
@@ -746,6 +768,8 @@ int64_t dd_plan_info(const dd_plan *plan, int what)
     case DD_INFO_CH: return t.shape.CH;
     case DD_INFO_NSTAGE: return t.nstage;
     case DD_INFO_PANEL: return t.panel;
+    case DD_INFO_HOST_CHUNKS: return plan->last_chunks;
+    case DD_INFO_HOST_TAPER: return plan->last_taper;
     default: return -1;
     }
 }

@@ -116,6 +116,7 @@ __global__ void __launch_bounds__(kThreads, 1) lds_kernel(uint32_t *sink, long l
     if (threadIdx.x == 0) cycles[blockIdx.x] = t1 - t0;
 }
 
+#ifdef DD_TUNING  // experiments of DESIGN.md section 10 (numbers: profiles/r02_peaks.md): libdd_tuning.so only
 // ---------------------------------------------------------------- tensor memory next to shared memory
 // MODE 0: tcgen05.ld.32x32b.x8 only; 1: the same interleaved with four LDS.64 per iteration (equal bytes)
 template <int MODE>
@@ -284,6 +285,7 @@ __global__ void __launch_bounds__(512, 1) hybrid_kernel(uint32_t *sink, long lon
     __syncthreads();
     if (threadIdx.x < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base));
 }
+#endif  // DD_TUNING
 
 struct Scratch {
     uint32_t *sink = nullptr;
@@ -331,6 +333,7 @@ int lds_rate(Scratch &s, double *out)
     return rc;
 }
 
+#ifdef DD_TUNING
 template <int MODE>
 int tmem_rate(Scratch &s, double *out)
 {
@@ -355,6 +358,8 @@ int hybrid_rate(Scratch &s, double *out)
     if (rc == DD_OK) *out = 512.0 * 256 * 8 * 2 * 33 / cyc;
     return rc;
 }
+
+#endif  // DD_TUNING
 
 // SM clock under load: cycles of a long lane-rate launch against its CUDA-event time
 int sm_clock_mhz(Scratch &s, double *out)
@@ -419,11 +424,13 @@ extern "C" int dd_probe(int what, double *value)
     case DD_PROBE_IMAD_HI: return lane_rate<DD_PROBE_IMAD_HI>(s, value);
     case DD_PROBE_IDP4A: return lane_rate<DD_PROBE_IDP4A>(s, value);
     case DD_PROBE_SHF: return lane_rate<DD_PROBE_SHF>(s, value);
+#ifdef DD_TUNING
     case DD_PROBE_TMEM_LD: return tmem_rate<0>(s, value);
     case DD_PROBE_TMEM_LD_WITH_LDS: return tmem_rate<1>(s, value);
     case DD_PROBE_F32_ADDS_SMEM_ONLY: return hybrid_rate<0, true>(s, value);
     case DD_PROBE_F32_ADDS_TMEM_4_OF_8: return hybrid_rate<4, true>(s, value);
     case DD_PROBE_F32_ADDS_TMEM_4_OF_8_NO_FILL: return hybrid_rate<4, false>(s, value);
+#endif
     default: return DD_ERR_INVALID_ARG;
     }
 }

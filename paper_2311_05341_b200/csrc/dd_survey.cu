@@ -42,6 +42,13 @@ size_t block_bytes(int dtype, int nchans, int64_t nsamps)
     return dtype == DD_U4 ? n / 2 : n * (dtype == DD_U8 ? 1 : (dtype == DD_U16 ? 2 : 4));
 }
 
+// the survey's buffers and plans live on the device that was current at dd_survey_create (dd.h, dd_execute)
+bool on_survey_device(const dd_survey *s)
+{
+    int cur = -1;
+    return cudaGetDevice(&cur) == cudaSuccess && (s->device < 0 || cur == s->device);
+}
+
 void *binned_block(const dd_survey *s, int factor)
 {
     for (size_t i = 0; i < s->bin_factor.size(); ++i)
@@ -146,12 +153,14 @@ int dd_survey_range_dtype(const dd_survey *s, int range)
 int dd_survey_execute(dd_survey *s, const void *d_in, void *const *d_out, void *cuda_stream)
 {
     if (!s || !d_in || !d_out) return DD_ERR_INVALID_ARG;
+    if (!on_survey_device(s)) return DD_ERR_INVALID_ARG;
     return run_ranges(s, d_in, nullptr, d_out, cuda_stream);
 }
 
 int dd_survey_execute_tm(dd_survey *s, const void *d_in_tm, void *const *d_out, void *cuda_stream)
 {
     if (!s || !d_in_tm || !d_out) return DD_ERR_INVALID_ARG;
+    if (!on_survey_device(s)) return DD_ERR_INVALID_ARG;
     if (s->bin_factor.empty())  // no binned range: every plan reads the time-major block itself
         return run_ranges(s, nullptr, d_in_tm, d_out, cuda_stream);
     // binning works on channel-major rows: transpose once (PAPER.md:370 counts it in t_c), then

@@ -177,9 +177,10 @@ def test_full_output_parity(oracle, name):
 
 @pytest.mark.parametrize("name", ["headline", "lowfreq", "c3", "headline_u4"])
 def test_other_entry_points_equal_device_output_full_size(oracle, name):
-    """dd_execute_host / dd_execute_host_tm with NO chunk override (the default schedule: the
-    tapered 8-chunk pipeline with its two workspaces and two main streams -- what bench.py's e2e
-    leg times) and dd_execute_tm reproduce dd_execute's plane bit for bit; that plane is tied to
+    """dd_execute_host / dd_execute_host_tm with NO chunk override (the tapered 8-chunk pipeline with its
+    two workspaces and two main streams), dd_execute_host_async on its own default schedule, channel- and
+    time-major (what bench.py's e2e leg times; the schedule taken is asserted through dd_plan_info) and
+    dd_execute_tm reproduce dd_execute's plane bit for bit; that plane is tied to
     the oracle by sampled points here and as a whole in test_full_output_parity."""
     import torch
     B = _gpu()
@@ -205,6 +206,16 @@ def test_other_entry_points_equal_device_output_full_size(oracle, name):
         h_out = torch.full((plan.ndm, plan.out_len), -5, dtype=odt).pin_memory()
         plan.execute_host(h_in, h_out)
         assert torch.equal(h_out, out.cpu()), "dd_execute_host differs from dd_execute"
+        assert plan.info("HOST_TAPER") == 1 and plan.info("HOST_CHUNKS") == 8
+        # ---- the asynchronous form on ITS default schedule (what bench.py's e2e times): 4 equal chunks,
+        # the taper only for a block whose copies outlast its kernels (lowfreq)
+        side = torch.cuda.Stream()
+        h_out.fill_(-5)
+        plan.execute_host_async(h_in, h_out, side)
+        side.synchronize()
+        assert torch.equal(h_out, out.cpu()), "dd_execute_host_async differs from dd_execute"
+        assert plan.info("HOST_TAPER") == (1 if name == "lowfreq" else 0)
+        assert plan.info("HOST_CHUNKS") == (8 if name == "lowfreq" else 4)
         del h_in
         # ---- time-major: device path (fused transpose pre-pass) and host path
         if cfg.in_dtype == W.U4:
@@ -230,6 +241,11 @@ def test_other_entry_points_equal_device_output_full_size(oracle, name):
         h_out.fill_(-5)
         plan.execute_host_tm(h_tm, h_out)
         assert torch.equal(h_out, out.cpu()), "dd_execute_host_tm differs from dd_execute"
+        h_out.fill_(-5)
+        plan.execute_host_async(h_tm, h_out, side, time_major=True)
+        side.synchronize()
+        assert torch.equal(h_out, out.cpu()), "dd_execute_host_async (time-major) differs from dd_execute"
+        assert plan.info("HOST_TAPER") == (1 if name == "lowfreq" else 0)
     finally:
         plan.destroy()
 

@@ -875,6 +875,7 @@ def test_execute_host_async_two_blocks_in_flight(B, oracle, time_major):
         plans[0].execute_host_async(hin[2], houts[2], streams[0], time_major)   # same plan again: after block 0
         for s in streams:
             s.synchronize()
+        assert [p.info("HOST_CHUNKS") for p in plans] == [3, 3] and plans[0].info("HOST_TAPER") == 0
         tab = plans[0].shift_table()
         for x, h in zip(xs, houts):
             assert np.array_equal(h.numpy().view(np.uint32), oracle.dedisperse(x, tab, plans[0].out_len))
@@ -912,3 +913,35 @@ def test_one_plan_host_calls_from_different_streams_are_serialised(B, oracle):
             for h in houts:
                 h.zero_()
             d_out.zero_()
+
+
+def test_plan_refuses_a_call_from_another_current_device(B, oracle):
+    """An in-process multi-GPU caller (the 'replicas driven by the caller' of SURVEY.md 8(e)): a plan runs
+    on the device it was made on and refuses, with DD_ERR_INVALID_ARG and no launch, a call made while
+    another device is current; two plans on two devices from one process both equal the oracle."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs in one process")
+    rng = np.random.default_rng(3)
+    x = _rand_input(rng, np.uint8, 64, 6000)
+    dms = np.arange(16) * 2.0
+    outs, plans = [], []
+    try:
+        for dev in (0, 1):
+            torch.cuda.set_device(dev)
+            plan = B.Plan(64, 6000, 1500.0, -2.0, 64e-6, dms, B.DD_U8)
+            plans.append(plan)
+            d_in = torch.from_numpy(x).to("cuda:%d" % dev)
+            out = torch.zeros((plan.ndm, plan.out_len), dtype=torch.int32, device="cuda:%d" % dev)
+            plan.execute(d_in, out)
+            torch.cuda.synchronize(dev)
+            outs.append(out.cpu().numpy().view(np.uint32))
+        ref = oracle.dedisperse(x, plans[0].shift_table(), plans[0].out_len)
+        assert np.array_equal(outs[0], ref) and np.array_equal(outs[1], ref)
+        with pytest.raises(B.DDError) as e:      # device 1 is current, plan 0 lives on device 0
+            plans[0].execute(d_in, out)
+        assert e.value.status == B.DD_ERR_INVALID_ARG
+    finally:
+        torch.cuda.set_device(0)
+        for p in plans:
+            p.destroy()
